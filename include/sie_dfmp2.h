@@ -1,0 +1,134 @@
+/*
+ * sie_dfmp2.h — C ABI of libsie_dfmp2.so: fragment-projected density-fitted MP2 correlation energy of
+ * SIE embedding clusters on one NVIDIA B200 (sm_100a).
+ *
+ * What is computed (citations: /root/reference/PAPER.md line numbers; DESIGN.md §1 restates them):
+ *
+ *   B^P_{ia}    = sum_{mu nu} C_{mu i} (P|mu nu) C_{nu a}              DF form of the cluster integral
+ *                                                                     projection, Eq. S49 (L526)
+ *   (ia|jb)     = sum_P B^P_{ia} B^P_{jb}
+ *   t_{ij}^{ab} = (ia|jb) / (e_i + e_j - e_a - e_b)                    MP2 amplitudes, Eq. S15-S16 (L348-L351)
+ *   G_{i'i}     = sum_j sum_{ab} t_{i'j}^{ab} ( 2 (ia|jb) - (ib|ja) )  closed-shell 2t-t pattern, Eq. S17-S18/S22
+ *                                                                     (L355-L357, L390); only the first occupied
+ *                                                                     index is projected, Eq. S44/S50 (L501, L535)
+ *   E_frag      = sum_{i i'} P_frag[i][i'] G[i'][i] = Tr(P_frag G)     P_frag = C^f_{ii'}, Eq. S45/S59 (L505, L569)
+ *
+ * (P|mu nu) are already-fitted three-index factors (no metric is applied), restricted closed shell,
+ * real arithmetic, all nocc orbitals correlated, FP64 throughout.  G is NOT symmetric and is never
+ * symmetrised.  The orbital gap max(e_occ) < min(e_vir) is required (Eq. S16 denominators > 0).
+ *
+ * Conventions
+ *   - every function returns an int status (SIE_OK = 0); outputs are untouched on error.
+ *   - all matrices are row-major FP64.  The library never allocates device memory: the caller provides
+ *     one workspace (size reported by the plan / batch query), e.g. a torch uint8 tensor, and owns every
+ *     buffer.  Inputs are never modified and are not retained after the enqueued work completes.
+ *   - pointer arguments are DEVICE pointers unless the plan / batch was created with
+ *     SIE_FLAG_HOST_IO, in which case every data pointer (inputs and outputs, not the workspace) is a
+ *     HOST pointer (pinned memory recommended) and the library stages the copies itself on `cuda_stream`;
+ *     with SIE_FLAG_HOST_IO sie_dfmp2_energy / sie_dfmp2_batch synchronise the stream before returning.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls only enqueue
+ *     work unless stated otherwise.
+ *   - a plan is used by one host thread at a time; different plans are independent.
+ */
+#ifndef SIE_DFMP2_H
+#define SIE_DFMP2_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sie_dfmp2_plan_s* sie_dfmp2_plan_t;
+
+enum {
+    SIE_OK = 0,
+    SIE_EINVAL = 1,       /* bad size / null pointer / bad range */
+    SIE_ENOMEM = 2,       /* host allocation failed or workspace too small */
+    SIE_ECUDA = 3,        /* a CUDA runtime / driver call failed (see sie_dfmp2_last_cuda_error) */
+    SIE_ESTATE = 4,       /* call order violated (e.g. energy before the transform covered [0,naux)) */
+    SIE_EGAP = 5,         /* SIE_FLAG_VALIDATE only: max(e_occ) >= min(e_vir) */
+    SIE_EUNSUPPORTED = 6  /* no CUDA device of compute capability 10.x */
+};
+
+enum {
+    SIE_FLAG_VALIDATE = 1u,  /* energy/batch copy e_occ,e_vir to the host (synchronising) and check the gap */
+    SIE_FLAG_REFERENCE = 2u, /* use the simple FP64-FMA reference kernels (any nocc; slow; cross-check path) */
+    SIE_FLAG_HOST_IO = 4u    /* data pointers are HOST pointers; the library stages H2D/D2H copies */
+};
+
+/*
+ * 1. sie_dfmp2_plan — host only.  Validates the sizes, chooses tile configurations and the internal aux
+ *    sub-block, and reports the device workspace (bytes, 256-byte aligned base required) the caller must
+ *    pass to transform/energy.  The workspace holds B[a][i][P] between transform and energy.
+ *      nao >= nocc + nvir, nocc >= 1, nvir >= 1, naux >= 1; aux_block = rows of (P|mu nu) processed per
+ *      internal step (0 = auto).  nocc > 128 silently selects the reference kernels.
+ */
+int sie_dfmp2_plan(sie_dfmp2_plan_t* plan, int nao, int nocc, int nvir, int naux, int aux_block,
+                   unsigned flags, size_t* workspace_bytes);
+
+/*
+ * 2. sie_dfmp2_transform — AO->MO two-step half transform (steps A1+A2 of DESIGN.md) of the aux rows
+ *    [p0,p1); call repeatedly, in any order, until [0,naux) is covered exactly once (overlap -> SIE_EINVAL).
+ *      C_occ          [nao][nocc]   C_vir [nao][nvir]   (must be the same for every block of one plan)
+ *      L_packed_block [(p1-p0)][nao(nao+1)/2]: element (P,mu,nu), mu >= nu, at (P-p0)*npair + mu(mu+1)/2 + nu
+ *    Result: B^P_{ia} in the workspace (layout private to the library).
+ */
+int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_occ, const double* C_vir,
+                        const double* L_packed_block, int p0, int p1, void* cuda_stream);
+
+/*
+ * 3. sie_dfmp2_energy — fused pair stage (V, t, G never leave the chip) + projector/trace reduction
+ *    (steps A3-A6).   e_occ[nocc], e_vir[nvir], P_frag[nocc][nocc] = P[i][i'] (NULL = identity),
+ *    E_out: 1 double, G_out: [nocc][nocc] = G[i'][i] or NULL.  SIE_ESTATE if the transform has not
+ *    covered [0,naux).  May be called again with other e/P on the same B.
+ */
+int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir,
+                     const double* P_frag, double* E_out, double* G_out, void* cuda_stream);
+
+/*
+ * 4. sie_dfmp2_batch — many independent clusters (no contraction across clusters) in one
+ *    scheduled submission: per-cluster transforms, then ONE persistent pair kernel whose CTAs walk a
+ *    static, cost-balanced list of (cluster, tile) work items, then one reduction launch (step A7).
+ *      clusters: HOST array of descriptors (pointers device or host per SIE_FLAG_HOST_IO).
+ *      workspace_bytes == 0 or workspace == NULL: query only, *needed receives the required size.
+ */
+typedef struct {
+    int nao, nocc, nvir, naux;
+    const double* C_occ;    /* [nao][nocc] */
+    const double* C_vir;    /* [nao][nvir] */
+    const double* L_packed; /* [naux][nao(nao+1)/2] */
+    const double* e_occ;    /* [nocc] */
+    const double* e_vir;    /* [nvir] */
+    const double* P_frag;   /* [nocc][nocc] or NULL (identity) */
+    double* E_out;          /* 1 double */
+    double* G_out;          /* [nocc][nocc] or NULL */
+} sie_dfmp2_cluster_t;
+
+int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes,
+                    size_t* needed, unsigned flags, void* cuda_stream);
+
+/* Frees the host-side plan (never touches device memory). NULL is allowed. */
+int sie_dfmp2_destroy(sie_dfmp2_plan_t plan);
+
+/* Static string for a status code. */
+const char* sie_dfmp2_strerror(int status);
+
+/* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
+const char* sie_dfmp2_last_cuda_error(void);
+
+/* Number of kernels this library has launched since load (all threads); bench.py's gpu_launches. */
+unsigned long long sie_dfmp2_launch_count(void);
+
+/*
+ * Introspection for benchmarks/tests: fills info[0..n) with plan facts, returns how many exist.
+ *   0: pair-tile rows TM   1: pair-tile cols TN   2: virtual sub-blocks per tile side (ta)
+ *   3: nocc padded to 8 (o8)   4: number of pair tiles   5: persistent CTAs   6: internal aux sub-block
+ *   7: 1 if the reference kernels are selected
+ */
+int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SIE_DFMP2_H */

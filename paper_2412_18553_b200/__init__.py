@@ -1,0 +1,21 @@
+"""paper_2412_18553_b200 — B200-native fragment-projected DF-MP2 for SIE embedding clusters.
+
+The product is libsie_dfmp2.so (hand-written sm_100a CUDA behind the C ABI of include/sie_dfmp2.h);
+this package is its thin Python binding.  Nothing here computes on the CPU and nothing imports oracle/.
+"""
+from .binding import (  # noqa: F401
+    SIE_FLAG_HOST_IO,
+    SIE_FLAG_REFERENCE,
+    SIE_FLAG_VALIDATE,
+    ClusterSolver,
+    SieError,
+    alloc_workspace,
+    launch_count,
+    sie_dfmp2_batch,
+    sie_dfmp2_batch_query,
+    sie_dfmp2_destroy,
+    sie_dfmp2_energy,
+    sie_dfmp2_plan,
+    sie_dfmp2_plan_info,
+    sie_dfmp2_transform,
+)

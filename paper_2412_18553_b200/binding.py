@@ -1,0 +1,236 @@
+"""Thin Python binding of libsie_dfmp2.so (include/sie_dfmp2.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; torch is used for device memory
+(the workspace and the operand tensors) and streams.  There is no CPU fallback: a missing library or a
+missing GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import List, Optional, Sequence, Tuple
+
+import torch
+
+SIE_OK, SIE_EINVAL, SIE_ENOMEM, SIE_ECUDA, SIE_ESTATE, SIE_EGAP, SIE_EUNSUPPORTED = range(7)
+SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO = 1, 2, 4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsie_dfmp2.so")
+
+EXPORTS = (
+    "sie_dfmp2_plan",
+    "sie_dfmp2_transform",
+    "sie_dfmp2_energy",
+    "sie_dfmp2_batch",
+    "sie_dfmp2_destroy",
+    "sie_dfmp2_strerror",
+    "sie_dfmp2_last_cuda_error",
+    "sie_dfmp2_launch_count",
+    "sie_dfmp2_plan_info",
+)
+
+
+class SieError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = _lib().sie_dfmp2_strerror(status).decode()
+        if status == SIE_ECUDA:
+            msg += " — " + _lib().sie_dfmp2_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} (status {status})")
+
+
+class sie_dfmp2_cluster_t(ctypes.Structure):
+    _fields_ = [
+        ("nao", ctypes.c_int),
+        ("nocc", ctypes.c_int),
+        ("nvir", ctypes.c_int),
+        ("naux", ctypes.c_int),
+        ("C_occ", ctypes.c_void_p),
+        ("C_vir", ctypes.c_void_p),
+        ("L_packed", ctypes.c_void_p),
+        ("e_occ", ctypes.c_void_p),
+        ("e_vir", ctypes.c_void_p),
+        ("P_frag", ctypes.c_void_p),
+        ("E_out", ctypes.c_void_p),
+        ("G_out", ctypes.c_void_p),
+    ]
+
+
+_LIB = None
+
+
+def _lib() -> ctypes.CDLL:
+    """Load the CUDA library; raise loudly if it has not been built (no fallback exists)."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2412_18553_b200.build` "
+                "(nvcc, sm_100a). There is no CPU fallback."
+            )
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cu = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint
+        L.sie_dfmp2_plan.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, cu, ctypes.POINTER(ctypes.c_size_t)]
+        L.sie_dfmp2_plan.restype = ci
+        L.sie_dfmp2_transform.argtypes = [vp, vp, vp, vp, vp, ci, ci, vp]
+        L.sie_dfmp2_transform.restype = ci
+        L.sie_dfmp2_energy.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+        L.sie_dfmp2_energy.restype = ci
+        L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
+        L.sie_dfmp2_batch.restype = ci
+        L.sie_dfmp2_destroy.argtypes = [vp]
+        L.sie_dfmp2_destroy.restype = ci
+        L.sie_dfmp2_strerror.argtypes = [ci]
+        L.sie_dfmp2_strerror.restype = ctypes.c_char_p
+        L.sie_dfmp2_last_cuda_error.argtypes = []
+        L.sie_dfmp2_last_cuda_error.restype = ctypes.c_char_p
+        L.sie_dfmp2_launch_count.argtypes = []
+        L.sie_dfmp2_launch_count.restype = ctypes.c_ulonglong
+        L.sie_dfmp2_plan_info.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong), ci]
+        L.sie_dfmp2_plan_info.restype = ci
+        _LIB = L
+    return _LIB
+
+
+def _check(status: int, where: str) -> None:
+    if status != SIE_OK:
+        raise SieError(status, where)
+
+
+def _ptr(t: Optional[torch.Tensor], host: bool, name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name}: need a contiguous float64 tensor")
+    if host and t.is_cuda:
+        raise TypeError(f"{name}: SIE_FLAG_HOST_IO needs host tensors")
+    if not host and not t.is_cuda:
+        raise TypeError(f"{name}: need a CUDA tensor (or plan with SIE_FLAG_HOST_IO)")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return s.cuda_stream
+
+
+def launch_count() -> int:
+    return int(_lib().sie_dfmp2_launch_count())
+
+
+# ------------------------------------------------------------------------------------------------ C-ABI names
+def sie_dfmp2_plan(nao: int, nocc: int, nvir: int, naux: int, aux_block: int = 0, flags: int = 0) -> Tuple[int, int]:
+    """-> (plan handle, workspace bytes)."""
+    h = ctypes.c_void_p()
+    ws = ctypes.c_size_t()
+    _check(_lib().sie_dfmp2_plan(ctypes.byref(h), nao, nocc, nvir, naux, aux_block, flags, ctypes.byref(ws)), "sie_dfmp2_plan")
+    return h.value, ws.value
+
+
+def sie_dfmp2_transform(plan: int, workspace: torch.Tensor, C_occ, C_vir, L_packed_block, p0: int, p1: int, *, host=False, stream=None) -> None:
+    _check(
+        _lib().sie_dfmp2_transform(
+            plan, workspace.data_ptr(), _ptr(C_occ, host, "C_occ"), _ptr(C_vir, host, "C_vir"),
+            _ptr(L_packed_block, host, "L_packed_block"), p0, p1, _stream_ptr(stream)),
+        "sie_dfmp2_transform",
+    )
+
+
+def sie_dfmp2_energy(plan: int, workspace: torch.Tensor, e_occ, e_vir, P_frag, E_out, G_out, *, host=False, stream=None) -> None:
+    _check(
+        _lib().sie_dfmp2_energy(
+            plan, workspace.data_ptr(), _ptr(e_occ, host, "e_occ"), _ptr(e_vir, host, "e_vir"), _ptr(P_frag, host, "P_frag"),
+            _ptr(E_out, host, "E_out"), _ptr(G_out, host, "G_out"), _stream_ptr(stream)),
+        "sie_dfmp2_energy",
+    )
+
+
+def sie_dfmp2_destroy(plan: Optional[int]) -> None:
+    if plan:
+        _lib().sie_dfmp2_destroy(plan)
+
+
+def sie_dfmp2_plan_info(plan: int) -> dict:
+    buf = (ctypes.c_longlong * 8)()
+    n = _lib().sie_dfmp2_plan_info(plan, buf, 8)
+    keys = ("TM", "TN", "ta", "o8", "ntiles", "ncta", "aux_subblock", "reference")
+    return {k: int(buf[i]) for i, k in enumerate(keys[:n])}
+
+
+def _descs(clusters: Sequence[dict], host: bool) -> ctypes.Array:
+    arr = (sie_dfmp2_cluster_t * max(1, len(clusters)))()
+    for k, c in enumerate(clusters):
+        d = arr[k]
+        d.nao, d.nocc, d.nvir, d.naux = c["nao"], c["nocc"], c["nvir"], c["naux"]
+        for f in ("C_occ", "C_vir", "L_packed", "e_occ", "e_vir", "P_frag", "E_out", "G_out"):
+            setattr(d, f, _ptr(c.get(f), host, f))
+    return arr
+
+
+def sie_dfmp2_batch_query(clusters: Sequence[dict], flags: int = 0) -> int:
+    """Workspace bytes needed for this batch (sizes only are read)."""
+    arr = (sie_dfmp2_cluster_t * max(1, len(clusters)))()
+    for k, c in enumerate(clusters):
+        arr[k].nao, arr[k].nocc, arr[k].nvir, arr[k].naux = c["nao"], c["nocc"], c["nvir"], c["naux"]
+    need = ctypes.c_size_t()
+    _check(_lib().sie_dfmp2_batch(len(clusters), arr, None, 0, ctypes.byref(need), flags, None), "sie_dfmp2_batch(query)")
+    return need.value
+
+
+def sie_dfmp2_batch(clusters: Sequence[dict], workspace: torch.Tensor, flags: int = 0, *, stream=None) -> None:
+    """clusters: dicts with nao,nocc,nvir,naux and tensors C_occ,C_vir,L_packed,e_occ,e_vir,P_frag|None,E_out,G_out|None."""
+    host = bool(flags & SIE_FLAG_HOST_IO)
+    arr = _descs(clusters, host)
+    need = ctypes.c_size_t()
+    _check(
+        _lib().sie_dfmp2_batch(len(clusters), arr, workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                               ctypes.byref(need), flags, _stream_ptr(stream)),
+        "sie_dfmp2_batch",
+    )
+
+
+# ------------------------------------------------------------------------------------------------ convenience
+def alloc_workspace(nbytes: int, device="cuda") -> torch.Tensor:
+    """A 256-byte aligned uint8 device tensor (torch's caching allocator returns 512-byte aligned blocks)."""
+    t = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+    assert t.data_ptr() % 256 == 0
+    return t
+
+
+class ClusterSolver:
+    """One cluster: plan + workspace, transform fed by aux blocks, then energy.  Marshalling only."""
+
+    def __init__(self, nao: int, nocc: int, nvir: int, naux: int, aux_block: int = 0, flags: int = 0, device="cuda"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2412_18553_b200 needs a CUDA device (B200, sm_100a); there is no CPU path")
+        self.nao, self.nocc, self.nvir, self.naux, self.flags = nao, nocc, nvir, naux, flags
+        self.host = bool(flags & SIE_FLAG_HOST_IO)
+        self.plan, self.workspace_bytes = sie_dfmp2_plan(nao, nocc, nvir, naux, aux_block, flags)
+        self.workspace = alloc_workspace(self.workspace_bytes, device)
+        self.device = device
+
+    def info(self) -> dict:
+        return sie_dfmp2_plan_info(self.plan)
+
+    def transform(self, C_occ, C_vir, L_block, p0: int, p1: int, stream=None) -> None:
+        sie_dfmp2_transform(self.plan, self.workspace, C_occ, C_vir, L_block, p0, p1, host=self.host, stream=stream)
+
+    def energy(self, e_occ, e_vir, P_frag=None, want_G: bool = True, stream=None):
+        dev = "cpu" if self.host else self.device
+        E = torch.empty(1, dtype=torch.float64, device=dev)
+        G = torch.empty(self.nocc, self.nocc, dtype=torch.float64, device=dev) if want_G else None
+        if self.host:
+            E, G = E.pin_memory(), (G.pin_memory() if G is not None else None)
+        sie_dfmp2_energy(self.plan, self.workspace, e_occ, e_vir, P_frag, E, G, host=self.host, stream=stream)
+        return E, G
+
+    def close(self) -> None:
+        sie_dfmp2_destroy(self.plan)
+        self.plan = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

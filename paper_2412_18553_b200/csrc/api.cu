@@ -1,0 +1,726 @@
+// api.cu — the C-ABI boundary of libsie_dfmp2.so (include/sie_dfmp2.h): planning, workspace layout,
+// tensor-map encoding, the static (cluster, tile) schedule, and the launch sequences.
+#include <algorithm>
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/sie_dfmp2.h"
+#include "sie_common.cuh"
+#include "sie_internal.h"
+
+namespace sie {
+
+// ------------------------------------------------------------------------------------------------ bookkeeping
+static std::atomic<unsigned long long> g_launches{0};
+static thread_local std::string g_last_error;
+
+void note_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+int set_cuda_error_text(const char* s) {
+    g_last_error = s ? s : "";
+    return SIE_ECUDA;
+}
+int set_cuda_error(cudaError_t e) {
+    g_last_error = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e);
+    return SIE_ECUDA;
+}
+#define SIE_CUDA(call)                                   \
+    do {                                                 \
+        cudaError_t e__ = (call);                        \
+        if (e__ != cudaSuccess) return set_cuda_error(e__); \
+    } while (0)
+#define SIE_TRY(call)                  \
+    do {                               \
+        int rc__ = (call);             \
+        if (rc__ != SIE_OK) return rc__; \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------ tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+int make_tensor_map_3d(CUtensorMap* out, const double* base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t stride1_bytes,
+                       uint64_t stride2_bytes, uint32_t b0, uint32_t b1, uint32_t b2) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return set_cuda_error_text("cuTensorMapEncodeTiled entry point not available");
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {stride1_bytes, stride2_bytes};
+    cuuint32_t box[3] = {b0, b1, b2};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char buf[256];
+        snprintf(buf, sizeof buf,
+                 "cuTensorMapEncodeTiled failed (%d): dims {%llu,%llu,%llu} strides {%llu,%llu} box {%u,%u,%u} base %p", (int)r,
+                 (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2, (unsigned long long)stride1_bytes,
+                 (unsigned long long)stride2_bytes, b0, b1, b2, (const void*)base);
+        return set_cuda_error_text(buf);
+    }
+    return SIE_OK;
+}
+
+static int query_num_sms() {
+    static int sms = -1;
+    if (sms < 0) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            sms = n;
+        else {
+            (void)cudaGetLastError();
+            return 148;  // planning without a device (CPU-only host): B200 value
+        }
+    }
+    return sms;
+}
+
+static int check_device() {
+    static int ok = -1;
+    if (ok < 0) {
+        int dev = 0, major = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e != cudaSuccess) return set_cuda_error(e);
+        ok = (major == 10) ? 1 : 0;
+    }
+    return ok == 1 ? SIE_OK : SIE_EUNSUPPORTED;
+}
+
+}  // namespace sie
+
+using namespace sie;
+
+// ------------------------------------------------------------------------------------------------ plan
+struct sie_dfmp2_plan_s {
+    int nao = 0, o = 0, v = 0, naux = 0;
+    unsigned flags = 0;
+    bool ref = false;
+    int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, nblk = 0, pblk = 0, ncta = 0, kp = 1, num_sms = 148;
+    size_t npair = 0;
+    std::vector<PairTile> tiles;  // cluster field = 0; rewritten when used inside a batch
+    double tile_cost = 0;         // relative cost of one tile (for batch ordering)
+    // workspace offsets (bytes)
+    size_t off_B = 0, off_CoT = 0, off_CvT = 0, off_Lfull = 0, off_H = 0, off_gpart = 0, off_desc = 0, off_tiles = 0, off_rc = 0,
+           off_stage = 0, off_io = 0, off_refH = 0, off_refVj = 0, off_refG = 0, total = 0;
+    size_t gpart_bytes = 0, stage_buf_bytes = 0;
+    // io sub-offsets (doubles, relative to off_io)
+    size_t io_Cocc = 0, io_Cvir = 0, io_eo = 0, io_ev = 0, io_P = 0, io_E = 0, io_G = 0, io_doubles = 0;
+    // state
+    std::vector<std::pair<int, int>> covered;
+    long long covered_rows = 0;
+    const void* c_ready_ws = nullptr;  // workspace for which the transposed coefficient copies are valid
+    const double* dC_occ = nullptr;    // device pointers of the coefficients used by the transform
+    const double* dC_vir = nullptr;
+    // HOST_IO copy pipeline
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr}, ev_fork = nullptr;
+    int stage_turn = 0;
+};
+
+namespace {
+
+struct Carver {
+    size_t off = 0;
+    size_t take(size_t bytes) {
+        size_t r = off;
+        off = align_up(off + bytes, 256);
+        return r;
+    }
+};
+
+void build_tiles(int nblk, std::vector<PairTile>& out) {
+    // upper triangle bi <= bj, enumerated in column groups of S blocks so that the ~148 tiles in flight
+    // share a dozen A panels and a dozen B panels (L2 reuse of the streamed operands)
+    const int S = 12;
+    out.clear();
+    out.reserve((size_t)nblk * (nblk + 1) / 2);
+    for (int J0 = 0; J0 < nblk; J0 += S) {
+        const int J1 = std::min(nblk, J0 + S);
+        for (int bi = 0; bi < J1; ++bi)
+            for (int bj = std::max(bi, J0); bj < J1; ++bj) out.push_back(PairTile{0, (unsigned short)bi, (unsigned short)bj});
+    }
+}
+
+int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags, bool carve_shared) {
+    if (nao < 1 || nocc < 1 || nvir < 1 || naux < 1 || aux_block < 0) return SIE_EINVAL;
+    if ((long long)nocc + nvir > nao) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO)) return SIE_EINVAL;
+    p.nao = nao;
+    p.o = nocc;
+    p.v = nvir;
+    p.naux = naux;
+    p.flags = flags;
+    p.npair = (size_t)nao * (nao + 1) / 2;
+    p.num_sms = query_num_sms();
+    const PairGeom geo = pair_geom();
+    p.ref = (flags & SIE_FLAG_REFERENCE) || nocc > geo.TM;
+    p.nao_ld = (int)align_up((size_t)nao, 8);
+    p.naux_ld = (int)align_up((size_t)naux, 8);
+    p.o8 = (int)align_up((size_t)nocc, 8);
+    // internal aux sub-block
+    if (aux_block > 0) {
+        p.pblk = std::min(aux_block, naux);
+    } else if (p.ref) {
+        p.pblk = std::min(naux, 64);
+    } else {
+        const int nvb = (nao + 127) / 128;
+        int pb = (2 * p.num_sms + nvb - 1) / nvb;
+        const size_t per_p = (size_t)nao * p.nao_ld * 8;
+        const int cap = (int)std::max<size_t>(8, ((size_t)512 << 20) / per_p);
+        pb = std::max(8, std::min(std::min(pb, 128), cap));
+        pb = (pb + 7) / 8 * 8;
+        p.pblk = std::min(pb, naux);
+    }
+    if (!p.ref) {
+        if (nvir > 65535 * (geo.TM / p.o8 > 0 ? geo.TM / p.o8 : 1)) return SIE_EINVAL;
+        p.ta = std::max(1, geo.TM / p.o8);
+        p.nblk = (nvir + p.ta - 1) / p.ta;
+        build_tiles(p.nblk, p.tiles);
+        p.ncta = (int)std::min<size_t>((size_t)p.num_sms, p.tiles.size());
+        const int nt8 = p.o8 / 8;
+        p.kp = nt8 >= geo.ncons ? 1 : geo.ncons / nt8;
+        p.gpart_bytes = (size_t)p.num_sms * p.kp * p.o8 * p.o8 * 8;  // sized for any CTA count up to num_sms
+        p.tile_cost = (double)geo.TM * geo.TN * naux + 4.0 * p.ta * p.ta * (double)p.o8 * p.o8 * p.o8;
+    }
+    // workspace
+    Carver c;
+    p.off_B = c.take((size_t)nvir * nocc * p.naux_ld * 8);
+    if (!p.ref)
+        p.off_gpart = c.take(p.gpart_bytes);
+    else
+        p.off_refG = c.take((size_t)nocc * nocc * 8);
+    if (carve_shared) {
+        if (!p.ref) {
+            p.off_CoT = c.take((size_t)nocc * p.nao_ld * 8);
+            p.off_CvT = c.take((size_t)nvir * p.nao_ld * 8);
+            p.off_Lfull = c.take((size_t)p.pblk * nao * p.nao_ld * 8);
+            p.off_H = c.take((size_t)nocc * p.pblk * p.nao_ld * 8);
+            p.off_desc = c.take(sizeof(PairCluster));
+            p.off_tiles = c.take(p.tiles.size() * sizeof(PairTile));
+        } else {
+            p.off_refH = c.take((size_t)p.pblk * nocc * nao * 8);
+            p.off_refVj = c.take(ref_vj_bytes(nocc, nvir));
+        }
+        p.off_rc = c.take(sizeof(ReduceCluster));
+        if (flags & SIE_FLAG_HOST_IO) {
+            p.stage_buf_bytes = align_up((size_t)p.pblk * p.npair * 8, 256);
+            p.off_stage = c.take(2 * p.stage_buf_bytes);
+            size_t d = 0;
+            p.io_Cocc = d, d += (size_t)nao * nocc;
+            p.io_Cvir = d, d += (size_t)nao * nvir;
+            p.io_eo = d, d += nocc;
+            p.io_ev = d, d += nvir;
+            p.io_P = d, d += (size_t)nocc * nocc;
+            p.io_E = d, d += 2;
+            p.io_G = d, d += (size_t)nocc * nocc;
+            p.io_doubles = d;
+            p.off_io = c.take(d * 8);
+        }
+    }
+    p.total = c.off;
+    return SIE_OK;
+}
+
+int ensure_copy_pipeline(sie_dfmp2_plan_s& p) {
+    if (p.copy_stream) return SIE_OK;
+    SIE_CUDA(cudaStreamCreateWithFlags(&p.copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        SIE_CUDA(cudaEventCreateWithFlags(&p.ev_ready[i], cudaEventDisableTiming));
+        SIE_CUDA(cudaEventCreateWithFlags(&p.ev_consumed[i], cudaEventDisableTiming));
+    }
+    SIE_CUDA(cudaEventCreateWithFlags(&p.ev_fork, cudaEventDisableTiming));
+    return SIE_OK;
+}
+
+struct Scratch {  // shared transform scratch (device pointers)
+    double *CoT, *CvT, *Lfull, *H, *refH;
+    unsigned char* stage;  // HOST_IO: 2 staging buffers
+    size_t stage_buf_bytes;
+};
+
+// Transform of aux rows [p0,p1) into Bmat ([v][o][naux_ld]).  L points at row p0 (device, or host when host_L).
+int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, double* Bmat, const Scratch& sc, const double* dC_occ,
+                   const double* dC_vir, const double* L, bool host_L, int p0, int p1, cudaStream_t st) {
+    const int nao = p.nao, o = p.o, v = p.v;
+    if (p.ref) {
+        for (int q0 = p0; q0 < p1; q0 += p.pblk) {
+            const int q1 = std::min(p1, q0 + p.pblk);
+            const double* Lq = L + (size_t)(q0 - p0) * p.npair;
+            if (host_L) {
+                SIE_CUDA(cudaMemcpyAsync(sc.stage, Lq, (size_t)(q1 - q0) * p.npair * 8, cudaMemcpyHostToDevice, st));
+                Lq = reinterpret_cast<const double*>(sc.stage);
+            }
+            SIE_TRY(ref_transform(dC_occ, dC_vir, Lq, nao, o, v, q0, q1, sc.refH, Bmat, p.naux_ld, st));
+        }
+        return SIE_OK;
+    }
+    const int tm1 = gemm_tm_for(o), tm2 = gemm_tm_for(v);
+    const int nvb = (nao + 127) / 128;
+    const int kblocks = (nao + 7) / 8;
+    CUtensorMap mapCo, mapCv;
+    SIE_TRY(make_tensor_map_3d(&mapCo, sc.CoT, nao, o, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * o, 8, tm1, 1));
+    SIE_TRY(make_tensor_map_3d(&mapCv, sc.CvT, nao, v, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * v, 8, tm2, 1));
+    if (host_L) SIE_TRY(ensure_copy_pipeline(pipe_owner));
+    for (int q0 = p0; q0 < p1; q0 += p.pblk) {
+        const int q1 = std::min(p1, q0 + p.pblk), pb = q1 - q0;
+        const double* Lq = L + (size_t)(q0 - p0) * p.npair;
+        if (host_L) {
+            // double-buffered H2D staging on a side stream, ordered against the unpack that consumes each buffer
+            sie_dfmp2_plan_s& po = pipe_owner;
+            const int buf = po.stage_turn & 1;
+            po.stage_turn++;
+            unsigned char* dst = sc.stage + (size_t)buf * sc.stage_buf_bytes;
+            SIE_CUDA(cudaEventRecord(po.ev_fork, st));  // staging must not start before earlier work on `st` that owns the workspace
+            SIE_CUDA(cudaStreamWaitEvent(po.copy_stream, po.ev_fork, 0));
+            SIE_CUDA(cudaStreamWaitEvent(po.copy_stream, po.ev_consumed[buf], 0));
+            SIE_CUDA(cudaMemcpyAsync(dst, Lq, (size_t)pb * p.npair * 8, cudaMemcpyHostToDevice, po.copy_stream));
+            SIE_CUDA(cudaEventRecord(po.ev_ready[buf], po.copy_stream));
+            SIE_CUDA(cudaStreamWaitEvent(st, po.ev_ready[buf], 0));
+            SIE_TRY(launch_unpack(reinterpret_cast<const double*>(dst), pb, nao, sc.Lfull, p.nao_ld, st));
+            SIE_CUDA(cudaEventRecord(po.ev_consumed[buf], st));
+        } else {
+            SIE_TRY(launch_unpack(Lq, pb, nao, sc.Lfull, p.nao_ld, st));
+        }
+        // A1: H[i][P][nu] = sum_mu CoT[i][mu] * Lfull[P][nu][mu]
+        CUtensorMap mapL, mapH;
+        SIE_TRY(make_tensor_map_3d(&mapL, sc.Lfull, nao, nao, pb, (uint64_t)p.nao_ld * 8, (uint64_t)nao * p.nao_ld * 8, 8, 128, 1));
+        GemmOut o1;
+        o1.base = sc.H;
+        o1.ld_m = (long long)pb * p.nao_ld;
+        o1.M = o;
+        o1.inner = nvb * 128;
+        o1.valid_inner = nao;
+        o1.stride_outer = p.nao_ld;
+        o1.n_lin_total = (long long)pb * nvb * 128;
+        SIE_TRY(launch_gemm_tn(tm1, mapCo, mapL, 1, pb * nvb, nvb, (long long)nvb * 128, kblocks, o1, p.num_sms, st));
+        // A2: B[a][i][q0+P] = sum_nu CvT[a][nu] * H[(i,P)][nu]
+        SIE_TRY(make_tensor_map_3d(&mapH, sc.H, nao, (uint64_t)o * pb, 1, (uint64_t)p.nao_ld * 8,
+                                   (uint64_t)p.nao_ld * 8 * o * pb, 8, 128, 1));
+        GemmOut o2;
+        o2.base = Bmat + q0;
+        o2.ld_m = (long long)o * p.naux_ld;
+        o2.M = v;
+        o2.inner = pb;
+        o2.valid_inner = pb;
+        o2.stride_outer = p.naux_ld;
+        o2.n_lin_total = (long long)o * pb;
+        const int m_tiles = (v + tm2 - 1) / tm2, n_tiles = (int)(((long long)o * pb + 127) / 128);
+        SIE_TRY(launch_gemm_tn(tm2, mapCv, mapH, m_tiles, n_tiles, n_tiles, 0, kblocks, o2, p.num_sms, st));
+    }
+    return SIE_OK;
+}
+
+int prepare_coeffs(sie_dfmp2_plan_s& p, const Scratch& sc, const double* dC_occ, const double* dC_vir, cudaStream_t st) {
+    if (p.ref) return SIE_OK;
+    SIE_TRY(launch_transpose(dC_occ, p.nao, p.o, sc.CoT, p.nao_ld, st));
+    SIE_TRY(launch_transpose(dC_vir, p.nao, p.v, sc.CvT, p.nao_ld, st));
+    return SIE_OK;
+}
+
+int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const double* de_occ, const double* de_vir, double* gpart,
+                      int kp, PairCluster& d) {
+    std::memset(&d, 0, sizeof d);
+    SIE_TRY(make_tensor_map_3d(&d.map, Bmat, p.naux, p.o, p.v, (uint64_t)p.naux_ld * 8, (uint64_t)p.o * p.naux_ld * 8, 8, p.o8, p.ta));
+    d.e_occ = de_occ;
+    d.e_vir = de_vir;
+    d.gpart = gpart;
+    d.o = p.o;
+    d.v = p.v;
+    d.o8 = p.o8;
+    d.ta = p.ta;
+    d.kblocks = (p.naux + 7) / 8;
+    d.kp = kp;
+    d.tx_bytes = 2u * 8u * (uint32_t)p.o8 * (uint32_t)p.ta * 8u;
+    return SIE_OK;
+}
+
+int check_gap_host(const double* e_occ, const double* e_vir, int o, int v) {
+    double mo = e_occ[0], mv = e_vir[0];
+    for (int i = 1; i < o; ++i) mo = std::max(mo, e_occ[i]);
+    for (int a = 1; a < v; ++a) mv = std::min(mv, e_vir[a]);
+    return (mo < mv) ? SIE_OK : SIE_EGAP;  // NaN compares false -> SIE_EGAP
+}
+
+bool add_interval(std::vector<std::pair<int, int>>& cov, int p0, int p1) {
+    for (auto& iv : cov)
+        if (p0 < iv.second && iv.first < p1) return false;
+    cov.emplace_back(p0, p1);
+    return true;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+int sie_dfmp2_plan(sie_dfmp2_plan_t* plan, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags,
+                   size_t* workspace_bytes) {
+    if (!plan || !workspace_bytes) return SIE_EINVAL;
+    sie_dfmp2_plan_s* p = new (std::nothrow) sie_dfmp2_plan_s();
+    if (!p) return SIE_ENOMEM;
+    int rc;
+    try {
+        rc = plan_init(*p, nao, nocc, nvir, naux, aux_block, flags, true);
+    } catch (const std::bad_alloc&) {
+        rc = SIE_ENOMEM;
+    }
+    if (rc != SIE_OK) {
+        delete p;
+        return rc;
+    }
+    *plan = p;
+    *workspace_bytes = p->total;
+    return SIE_OK;
+}
+
+int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_occ, const double* C_vir,
+                        const double* L_packed_block, int p0, int p1, void* cuda_stream) {
+    if (!plan || !workspace || !C_occ || !C_vir || !L_packed_block) return SIE_EINVAL;
+    sie_dfmp2_plan_s& p = *plan;
+    if (p0 < 0 || p1 > p.naux || p0 >= p1) return SIE_EINVAL;
+    if (reinterpret_cast<uintptr_t>(workspace) & 255) return SIE_EINVAL;
+    SIE_TRY(check_device());
+    for (auto& iv : p.covered)
+        if (p0 < iv.second && iv.first < p1) return SIE_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    const bool host = p.flags & SIE_FLAG_HOST_IO;
+    Scratch sc{};
+    sc.CoT = reinterpret_cast<double*>(ws + p.off_CoT);
+    sc.CvT = reinterpret_cast<double*>(ws + p.off_CvT);
+    sc.Lfull = reinterpret_cast<double*>(ws + p.off_Lfull);
+    sc.H = reinterpret_cast<double*>(ws + p.off_H);
+    sc.refH = reinterpret_cast<double*>(ws + p.off_refH);
+    sc.stage = ws + p.off_stage;
+    sc.stage_buf_bytes = p.stage_buf_bytes;
+    if (p.c_ready_ws != workspace || p.covered.empty()) {
+        const double *dCo = C_occ, *dCv = C_vir;
+        if (host) {
+            double* io = reinterpret_cast<double*>(ws + p.off_io);
+            SIE_CUDA(cudaMemcpyAsync(io + p.io_Cocc, C_occ, (size_t)p.nao * p.o * 8, cudaMemcpyHostToDevice, st));
+            SIE_CUDA(cudaMemcpyAsync(io + p.io_Cvir, C_vir, (size_t)p.nao * p.v * 8, cudaMemcpyHostToDevice, st));
+            dCo = io + p.io_Cocc;
+            dCv = io + p.io_Cvir;
+        }
+        SIE_TRY(prepare_coeffs(p, sc, dCo, dCv, st));
+        p.dC_occ = dCo;
+        p.dC_vir = dCv;
+        p.c_ready_ws = workspace;
+    }
+    SIE_TRY(transform_rows(p, p, reinterpret_cast<double*>(ws + p.off_B), sc, p.dC_occ, p.dC_vir, L_packed_block, host, p0, p1, st));
+    add_interval(p.covered, p0, p1);
+    p.covered_rows += p1 - p0;
+    return SIE_OK;
+}
+
+int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, const double* P_frag,
+                     double* E_out, double* G_out, void* cuda_stream) {
+    if (!plan || !workspace || !e_occ || !e_vir || !E_out) return SIE_EINVAL;
+    sie_dfmp2_plan_s& p = *plan;
+    if (p.covered_rows != p.naux || p.c_ready_ws != workspace) return SIE_ESTATE;
+    SIE_TRY(check_device());
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    const bool host = p.flags & SIE_FLAG_HOST_IO;
+    const int o = p.o, v = p.v;
+
+    const double *de_occ = e_occ, *de_vir = e_vir, *dP = P_frag;
+    double *dE = E_out, *dG = G_out;
+    double* io = reinterpret_cast<double*>(ws + p.off_io);
+    if (host) {
+        if (p.flags & SIE_FLAG_VALIDATE) SIE_TRY(check_gap_host(e_occ, e_vir, o, v));
+        SIE_CUDA(cudaMemcpyAsync(io + p.io_eo, e_occ, (size_t)o * 8, cudaMemcpyHostToDevice, st));
+        SIE_CUDA(cudaMemcpyAsync(io + p.io_ev, e_vir, (size_t)v * 8, cudaMemcpyHostToDevice, st));
+        de_occ = io + p.io_eo;
+        de_vir = io + p.io_ev;
+        if (P_frag) {
+            SIE_CUDA(cudaMemcpyAsync(io + p.io_P, P_frag, (size_t)o * o * 8, cudaMemcpyHostToDevice, st));
+            dP = io + p.io_P;
+        }
+        dE = io + p.io_E;
+        dG = G_out ? io + p.io_G : nullptr;
+    } else if (p.flags & SIE_FLAG_VALIDATE) {
+        std::vector<double> he(o + v);
+        SIE_CUDA(cudaMemcpyAsync(he.data(), e_occ, (size_t)o * 8, cudaMemcpyDeviceToHost, st));
+        SIE_CUDA(cudaMemcpyAsync(he.data() + o, e_vir, (size_t)v * 8, cudaMemcpyDeviceToHost, st));
+        SIE_CUDA(cudaStreamSynchronize(st));
+        SIE_TRY(check_gap_host(he.data(), he.data() + o, o, v));
+    }
+
+    const double* Bmat = reinterpret_cast<const double*>(ws + p.off_B);
+    ReduceCluster rc{};
+    rc.P = dP;
+    rc.E_out = dE;
+    rc.G_out = dG;
+    rc.o = o;
+    if (p.ref) {
+        double* G = reinterpret_cast<double*>(ws + p.off_refG);
+        SIE_TRY(ref_pair(Bmat, o, v, p.naux, p.naux_ld, de_occ, de_vir, reinterpret_cast<double*>(ws + p.off_refVj), G, st));
+        rc.gpart = G;
+        rc.o8 = o;
+        rc.nslots = 1;
+    } else {
+        double* gpart = reinterpret_cast<double*>(ws + p.off_gpart);
+        PairCluster pc;
+        SIE_TRY(fill_pair_cluster(p, Bmat, de_occ, de_vir, gpart, p.kp, pc));
+        SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
+        SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+        SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)p.ncta * p.kp * p.o8 * p.o8 * 8, st));
+        SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc), reinterpret_cast<const PairTile*>(ws + p.off_tiles),
+                            (int)p.tiles.size(), p.ncta, st));
+        rc.gpart = gpart;
+        rc.o8 = p.o8;
+        rc.nslots = p.ncta * p.kp;
+    }
+    SIE_CUDA(cudaMemcpyAsync(ws + p.off_rc, &rc, sizeof rc, cudaMemcpyHostToDevice, st));
+    SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
+    if (host) {
+        SIE_CUDA(cudaMemcpyAsync(E_out, dE, 8, cudaMemcpyDeviceToHost, st));
+        if (G_out) SIE_CUDA(cudaMemcpyAsync(G_out, dG, (size_t)o * o * 8, cudaMemcpyDeviceToHost, st));
+        SIE_CUDA(cudaStreamSynchronize(st));
+    }
+    return SIE_OK;
+}
+
+int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes, size_t* needed,
+                    unsigned flags, void* cuda_stream) {
+    if (ncluster < 0 || (ncluster > 0 && !clusters)) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO)) return SIE_EINVAL;
+    const bool host = flags & SIE_FLAG_HOST_IO;
+    const bool query = (workspace == nullptr || workspace_bytes == 0);
+    if (query && !needed) return SIE_EINVAL;
+    try {
+        // ---- per-cluster plans (B + partial-G regions) and shared scratch sized for the largest cluster
+        std::vector<sie_dfmp2_plan_s> plans(ncluster);
+        Carver c;
+        std::vector<size_t> off_cl(ncluster), off_io(ncluster);
+        size_t max_CoT = 0, max_CvT = 0, max_Lfull = 0, max_H = 0, max_refH = 0, max_refVj = 0, max_stage = 0, ntiles_total = 0;
+        for (int k = 0; k < ncluster; ++k) {
+            const sie_dfmp2_cluster_t& cl = clusters[k];
+            if (!query && (!cl.C_occ || !cl.C_vir || !cl.L_packed || !cl.e_occ || !cl.e_vir || !cl.E_out)) return SIE_EINVAL;
+            sie_dfmp2_plan_s& p = plans[k];
+            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~SIE_FLAG_HOST_IO, false));
+            off_cl[k] = c.take(p.total);
+            if (!p.ref) {
+                max_CoT = std::max(max_CoT, (size_t)p.o * p.nao_ld * 8);
+                max_CvT = std::max(max_CvT, (size_t)p.v * p.nao_ld * 8);
+                max_Lfull = std::max(max_Lfull, (size_t)p.pblk * p.nao * p.nao_ld * 8);
+                max_H = std::max(max_H, (size_t)p.o * p.pblk * p.nao_ld * 8);
+                ntiles_total += p.tiles.size();
+            } else {
+                max_refH = std::max(max_refH, (size_t)p.pblk * p.o * p.nao * 8);
+                max_refVj = std::max(max_refVj, ref_vj_bytes(p.o, p.v));
+            }
+            max_stage = std::max(max_stage, align_up((size_t)p.pblk * p.npair * 8, 256));
+            if (host) {
+                size_t d = (size_t)p.nao * p.o + (size_t)p.nao * p.v + p.o + p.v + 2 * (size_t)p.o * p.o + 2;
+                off_io[k] = c.take(d * 8);
+            }
+        }
+        const size_t off_CoT = c.take(max_CoT), off_CvT = c.take(max_CvT), off_Lfull = c.take(max_Lfull), off_H = c.take(max_H);
+        const size_t off_refH = c.take(max_refH), off_refVj = c.take(max_refVj);
+        const size_t off_stage = host ? c.take(2 * max_stage) : 0;
+        const size_t off_desc = c.take((size_t)std::max(1, ncluster) * sizeof(PairCluster));
+        const size_t off_tiles = c.take(std::max<size_t>(1, ntiles_total) * sizeof(PairTile));
+        const size_t off_rc = c.take((size_t)std::max(1, ncluster) * sizeof(ReduceCluster));
+        const size_t total = c.off;
+        if (needed) *needed = total;
+        if (query) return SIE_OK;
+        if (workspace_bytes < total) return SIE_ENOMEM;
+        if (reinterpret_cast<uintptr_t>(workspace) & 255) return SIE_EINVAL;
+        if (ncluster == 0) return SIE_OK;
+        SIE_TRY(check_device());
+
+        cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+        unsigned char* ws = static_cast<unsigned char*>(workspace);
+        sie_dfmp2_plan_s pipe;  // owns the HOST_IO copy stream/events of this call
+        struct PipeGuard {
+            sie_dfmp2_plan_s& p;
+            ~PipeGuard() {
+                if (p.copy_stream) {
+                    cudaStreamSynchronize(p.copy_stream);
+                    for (int i = 0; i < 2; ++i) {
+                        cudaEventDestroy(p.ev_ready[i]);
+                        cudaEventDestroy(p.ev_consumed[i]);
+                    }
+                    cudaEventDestroy(p.ev_fork);
+                    cudaStreamDestroy(p.copy_stream);
+                    p.copy_stream = nullptr;
+                }
+            }
+        } guard{pipe};
+
+        Scratch sc{};
+        sc.CoT = reinterpret_cast<double*>(ws + off_CoT);
+        sc.CvT = reinterpret_cast<double*>(ws + off_CvT);
+        sc.Lfull = reinterpret_cast<double*>(ws + off_Lfull);
+        sc.H = reinterpret_cast<double*>(ws + off_H);
+        sc.refH = reinterpret_cast<double*>(ws + off_refH);
+        sc.stage = ws + off_stage;
+        sc.stage_buf_bytes = max_stage;
+
+        std::vector<PairCluster> descs(ncluster);
+        std::vector<ReduceCluster> rcs(ncluster);
+        std::vector<const double*> de_occ(ncluster), de_vir(ncluster);
+        std::vector<double*> dE(ncluster), dG(ncluster);
+        // ---- stage 1: per-cluster transforms (A1, A2)
+        for (int k = 0; k < ncluster; ++k) {
+            const sie_dfmp2_cluster_t& cl = clusters[k];
+            sie_dfmp2_plan_s& p = plans[k];
+            unsigned char* wk = ws + off_cl[k];
+            const double *dCo = cl.C_occ, *dCv = cl.C_vir, *dP = cl.P_frag;
+            de_occ[k] = cl.e_occ;
+            de_vir[k] = cl.e_vir;
+            dE[k] = cl.E_out;
+            dG[k] = cl.G_out;
+            if (host) {
+                if (flags & SIE_FLAG_VALIDATE) SIE_TRY(check_gap_host(cl.e_occ, cl.e_vir, p.o, p.v));
+                double* io = reinterpret_cast<double*>(ws + off_io[k]);
+                size_t d = 0;
+                auto up = [&](const double* src, size_t n) -> const double* {
+                    double* dst = io + d;
+                    d += n;
+                    return cudaMemcpyAsync(dst, src, n * 8, cudaMemcpyHostToDevice, st) == cudaSuccess ? dst : nullptr;
+                };
+                dCo = up(cl.C_occ, (size_t)p.nao * p.o);
+                dCv = up(cl.C_vir, (size_t)p.nao * p.v);
+                de_occ[k] = up(cl.e_occ, p.o);
+                de_vir[k] = up(cl.e_vir, p.v);
+                if (cl.P_frag) dP = up(cl.P_frag, (size_t)p.o * p.o);
+                if (!dCo || !dCv || !de_occ[k] || !de_vir[k] || (cl.P_frag && !dP)) return set_cuda_error(cudaGetLastError());
+                dE[k] = io + d;
+                d += 2;
+                dG[k] = cl.G_out ? io + d : nullptr;
+            } else if (flags & SIE_FLAG_VALIDATE) {
+                std::vector<double> he(p.o + p.v);
+                SIE_CUDA(cudaMemcpyAsync(he.data(), cl.e_occ, (size_t)p.o * 8, cudaMemcpyDeviceToHost, st));
+                SIE_CUDA(cudaMemcpyAsync(he.data() + p.o, cl.e_vir, (size_t)p.v * 8, cudaMemcpyDeviceToHost, st));
+                SIE_CUDA(cudaStreamSynchronize(st));
+                SIE_TRY(check_gap_host(he.data(), he.data() + p.o, p.o, p.v));
+            }
+            SIE_TRY(prepare_coeffs(p, sc, dCo, dCv, st));
+            SIE_TRY(transform_rows(p, pipe, reinterpret_cast<double*>(wk + p.off_B), sc, dCo, dCv, cl.L_packed, host, 0, p.naux, st));
+            rcs[k] = ReduceCluster{};
+            rcs[k].P = dP;
+            rcs[k].E_out = dE[k];
+            rcs[k].G_out = dG[k];
+            rcs[k].o = p.o;
+        }
+        // ---- stage 2: one persistent pair launch over all (cluster, tile) items, most expensive tiles first
+        std::vector<int> order;
+        for (int k = 0; k < ncluster; ++k)
+            if (!plans[k].ref) order.push_back(k);
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return plans[a].tile_cost > plans[b].tile_cost; });
+        const int ncta = (int)std::min<size_t>((size_t)plans[0].num_sms, std::max<size_t>(1, ntiles_total));
+        std::vector<PairTile> tiles;
+        tiles.reserve(ntiles_total);
+        for (int k : order) {
+            sie_dfmp2_plan_s& p = plans[k];
+            unsigned char* wk = ws + off_cl[k];
+            double* gpart = reinterpret_cast<double*>(wk + p.off_gpart);
+            SIE_TRY(fill_pair_cluster(p, reinterpret_cast<const double*>(wk + p.off_B), de_occ[k], de_vir[k], gpart, p.kp, descs[k]));
+            SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)ncta * p.kp * p.o8 * p.o8 * 8, st));
+            for (PairTile t : p.tiles) {
+                t.cluster = k;
+                tiles.push_back(t);
+            }
+            rcs[k].gpart = gpart;
+            rcs[k].o8 = p.o8;
+            rcs[k].nslots = ncta * p.kp;
+        }
+        if (!tiles.empty()) {
+            SIE_CUDA(cudaMemcpyAsync(ws + off_desc, descs.data(), descs.size() * sizeof(PairCluster), cudaMemcpyHostToDevice, st));
+            SIE_CUDA(cudaMemcpyAsync(ws + off_tiles, tiles.data(), tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+            SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
+                                (int)tiles.size(), ncta, st));
+        }
+        // reference-path clusters (nocc > 128 or SIE_FLAG_REFERENCE): per-j kernels, one cluster at a time
+        for (int k = 0; k < ncluster; ++k) {
+            sie_dfmp2_plan_s& p = plans[k];
+            if (!p.ref) continue;
+            unsigned char* wk = ws + off_cl[k];
+            double* G = reinterpret_cast<double*>(wk + p.off_refG);
+            SIE_TRY(ref_pair(reinterpret_cast<const double*>(wk + p.off_B), p.o, p.v, p.naux, p.naux_ld, de_occ[k], de_vir[k],
+                             reinterpret_cast<double*>(ws + off_refVj), G, st));
+            rcs[k].gpart = G;
+            rcs[k].o8 = p.o;
+            rcs[k].nslots = 1;
+        }
+        SIE_CUDA(cudaMemcpyAsync(ws + off_rc, rcs.data(), rcs.size() * sizeof(ReduceCluster), cudaMemcpyHostToDevice, st));
+        SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + off_rc), ncluster, st));
+        if (host) {
+            for (int k = 0; k < ncluster; ++k) {
+                SIE_CUDA(cudaMemcpyAsync(clusters[k].E_out, dE[k], 8, cudaMemcpyDeviceToHost, st));
+                if (clusters[k].G_out)
+                    SIE_CUDA(cudaMemcpyAsync(clusters[k].G_out, dG[k], (size_t)plans[k].o * plans[k].o * 8, cudaMemcpyDeviceToHost, st));
+            }
+            SIE_CUDA(cudaStreamSynchronize(st));
+        }
+        return SIE_OK;
+    } catch (const std::bad_alloc&) {
+        return SIE_ENOMEM;
+    }
+}
+
+int sie_dfmp2_destroy(sie_dfmp2_plan_t plan) {
+    if (!plan) return SIE_OK;
+    if (plan->copy_stream) {
+        cudaStreamSynchronize(plan->copy_stream);
+        for (int i = 0; i < 2; ++i) {
+            cudaEventDestroy(plan->ev_ready[i]);
+            cudaEventDestroy(plan->ev_consumed[i]);
+        }
+        cudaEventDestroy(plan->ev_fork);
+        cudaStreamDestroy(plan->copy_stream);
+    }
+    delete plan;
+    return SIE_OK;
+}
+
+const char* sie_dfmp2_strerror(int status) {
+    switch (status) {
+        case SIE_OK: return "success";
+        case SIE_EINVAL: return "invalid argument";
+        case SIE_ENOMEM: return "out of memory or workspace too small";
+        case SIE_ECUDA: return "CUDA error";
+        case SIE_ESTATE: return "invalid call order";
+        case SIE_EGAP: return "orbital gap violated: max(e_occ) >= min(e_vir)";
+        case SIE_EUNSUPPORTED: return "no compute-capability-10.x CUDA device";
+        default: return "unknown status";
+    }
+}
+
+const char* sie_dfmp2_last_cuda_error(void) { return g_last_error.c_str(); }
+
+unsigned long long sie_dfmp2_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n) {
+    if (!plan) return 0;
+    const PairGeom geo = pair_geom();
+    const long long vals[8] = {geo.TM, geo.TN, plan->ta, plan->o8, (long long)plan->tiles.size(), plan->ncta, plan->pblk, plan->ref ? 1 : 0};
+    for (int i = 0; i < n && i < 8; ++i)
+        if (info) info[i] = vals[i];
+    return 8;
+}
+
+}  // extern "C"

@@ -1,0 +1,74 @@
+// sie_internal.h — host-side launcher declarations shared by the translation units of libsie_dfmp2.so.
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace sie {
+
+// ---- transform.cu ------------------------------------------------------------------------------
+// out[c][r] = in[r][c] for r < rows, c < cols; out has leading dimension ld_out (>= rows).
+int launch_transpose(const double* in, int rows, int cols, double* out, int ld_out, cudaStream_t st);
+// packed lower triangles [np][nao(nao+1)/2] -> full symmetric [np][nao][ld] (ld >= nao)
+int launch_unpack(const double* Lp, int np, int nao, double* Lfull, int ld, cudaStream_t st);
+
+struct GemmOut {
+    double* base;          // output base pointer
+    long long ld_m;        // offset per row m
+    int M;                 // valid rows
+    int inner;             // n_lin -> (outer = n_lin / inner, rem = n_lin % inner)
+    int valid_inner;       // column valid iff rem < valid_inner
+    long long stride_outer;  // offset = outer * stride_outer + rem
+    long long n_lin_total;   // column valid iff n_lin < n_lin_total
+};
+// C = A * B^T with K-major operands described by 3-D tensor maps (box {8, rows, 1}); tile nb of the B operand
+// sits at coordinates (k, (nb % nb_inner) * TN, nb / nb_inner) and its first column has
+// n_lin = (nb / nb_inner) * inner_pad + (nb % nb_inner) * TN.
+// tm_sel picks the M-tile height: 16, 32, 64 or 128 (TN is always 128).
+int launch_gemm_tn(int tm_sel, const CUtensorMap& mapA, const CUtensorMap& mapB, int m_tiles, int n_tiles, int nb_inner,
+                   long long inner_pad, int kblocks, const GemmOut& out, int num_sms, cudaStream_t st);
+int gemm_tm_for(int m);  // smallest supported M-tile height covering min(m,128)
+
+// ---- pair.cu -----------------------------------------------------------------------------------
+struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (global memory)
+    CUtensorMap map;               // B as {naux, nocc, nvir}, box {8, o8, ta}
+    const double* e_occ;
+    const double* e_vir;
+    double* gpart;                 // partial-G slots of this cluster: [ncta][kp][o8*o8]
+    int o, v, o8, ta;
+    int kblocks;                   // ceil(naux / 8)
+    int kp;                        // epilogue K-split parts
+    uint32_t tx_bytes;             // bytes of both operand boxes of one stage
+    int pad_;
+};
+struct PairTile {                  // 8 bytes
+    int cluster;
+    unsigned short bi, bj;         // virtual-block indices, bi <= bj
+};
+struct PairGeom {                  // tile configuration facts for host-side planning
+    int TM, TN, ncons;
+};
+PairGeom pair_geom();
+size_t pair_smem_bytes();
+int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, cudaStream_t st);
+
+struct ReduceCluster {             // per cluster, device array
+    const double* gpart;           // [nslots][o8*o8]
+    const double* P;               // [o][o] or nullptr
+    double* E_out;                 // 1
+    double* G_out;                 // [o][o] or nullptr
+    int o, o8, nslots, pad_;
+};
+int launch_reduce(const ReduceCluster* d_rc, int ncluster, cudaStream_t st);
+
+// ---- ref_kernels.cu ----------------------------------------------------------------------------
+// Simple FP64-FMA kernels following the definition step by step (any nocc). B layout [v][o][naux_ld].
+int ref_transform(const double* C_occ, const double* C_vir, const double* Lp_block, int nao, int o, int v, int p0, int p1,
+                  double* H /*[(p1-p0)][o][nao]*/, double* B, int naux_ld, cudaStream_t st);
+int ref_pair(const double* B, int o, int v, int naux, int naux_ld, const double* e_occ, const double* e_vir,
+             double* Vj /*[o][v][v]*/, double* G /*[o][o]*/, cudaStream_t st);
+size_t ref_vj_bytes(int o, int v);
+
+}  // namespace sie

@@ -1,0 +1,95 @@
+"""C-ABI library: loads on a CPU-only host, exports every symbol include/sie_dfmp2.h declares,
+host-side planning/validation logic.  No compute calls (those are the -m gpu tests)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2412_18553_b200 as sie
+from paper_2412_18553_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_2412_18553_b200 import build
+
+    build.build()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "sie_dfmp2.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(sie_dfmp2_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = ctypes.CDLL(binding.LIB_PATH)
+    declared = _declared_symbols()
+    assert {"sie_dfmp2_plan", "sie_dfmp2_transform", "sie_dfmp2_energy", "sie_dfmp2_batch"} <= set(declared)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert set(binding.EXPORTS) == set(declared)
+
+
+def test_library_does_not_link_libcuda():
+    """It must load where no driver exists (this container): only the static runtime is linked."""
+    import subprocess
+
+    out = subprocess.run(["ldd", binding.LIB_PATH], capture_output=True, text=True).stdout
+    assert "libcuda.so" not in out
+
+
+def test_plan_is_host_only_and_reports_workspace():
+    plan, ws = sie.sie_dfmp2_plan(48, 8, 40, 160)
+    info = sie.sie_dfmp2_plan_info(plan)
+    assert info["TM"] == 128 and info["TN"] == 128 and info["o8"] == 8 and info["ta"] == 16
+    nblk = (40 + 15) // 16
+    assert info["ntiles"] == nblk * (nblk + 1) // 2 and info["reference"] == 0
+    assert ws >= 40 * 8 * 160 * 8  # at least B
+    sie.sie_dfmp2_destroy(plan)
+    # config 3: B alone is ~5 GB; 1080 virtual blocks -> 584k tiles
+    plan, ws = sie.sie_dfmp2_plan(1200, 120, 1080, 4800)
+    info = sie.sie_dfmp2_plan_info(plan)
+    assert info["ta"] == 1 and info["o8"] == 120 and info["ntiles"] == 1080 * 1081 // 2 and info["ncta"] == 148
+    assert 4.9e9 < ws < 7e9
+    sie.sie_dfmp2_destroy(plan)
+    # nocc > 128 -> reference kernels
+    plan, _ = sie.sie_dfmp2_plan(400, 130, 200, 300)
+    assert sie.sie_dfmp2_plan_info(plan)["reference"] == 1
+    sie.sie_dfmp2_destroy(plan)
+
+
+@pytest.mark.parametrize("args", [(0, 1, 1, 1), (10, 0, 5, 5), (10, 5, 0, 5), (10, 5, 5, 0), (9, 5, 5, 5), (10, 5, 5, 5, -1), (10, 5, 5, 5, 0, 64)])
+def test_plan_rejects_bad_sizes(args):
+    with pytest.raises(sie.SieError) as ei:
+        sie.sie_dfmp2_plan(*args)
+    assert ei.value.status == binding.SIE_EINVAL
+
+
+def test_batch_query_needs_no_gpu():
+    cl = [dict(nao=48, nocc=8, nvir=40, naux=160), dict(nao=144, nocc=16, nvir=128, naux=576)]
+    n1 = sie.sie_dfmp2_batch_query(cl[:1])
+    n2 = sie.sie_dfmp2_batch_query(cl)
+    assert 0 < n1 < n2
+    assert sie.sie_dfmp2_batch_query(cl, binding.SIE_FLAG_HOST_IO) > n2
+    assert sie.sie_dfmp2_batch_query([]) >= 0
+
+
+def test_strerror_and_launch_counter():
+    lib = binding._lib()
+    assert lib.sie_dfmp2_strerror(0) == b"success"
+    assert b"gap" in lib.sie_dfmp2_strerror(binding.SIE_EGAP)
+    assert sie.launch_count() >= 0
+
+
+def test_product_does_not_import_oracle():
+    """The CUDA path and the oracle share no code: no file of the package mentions the oracle module."""
+    pkg = os.path.join(ROOT, "paper_2412_18553_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "dfmp2_oracle" not in src, f
