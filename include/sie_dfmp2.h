@@ -54,7 +54,8 @@ enum {
 enum {
     SIE_FLAG_VALIDATE = 1u,  /* energy/batch copy e_occ,e_vir to the host (synchronising) and check the gap */
     SIE_FLAG_REFERENCE = 2u, /* use the simple FP64-FMA reference kernels (any nocc; slow; cross-check path) */
-    SIE_FLAG_HOST_IO = 4u    /* data pointers are HOST pointers; the library stages H2D/D2H copies */
+    SIE_FLAG_HOST_IO = 4u,   /* data pointers are HOST pointers; the library stages H2D/D2H copies */
+    SIE_FLAG_PROFILE = 8u    /* bracket every launch group with CUDA events; read with *_timing (below) */
 };
 
 /*
@@ -127,6 +128,27 @@ unsigned long long sie_dfmp2_launch_count(void);
  *   7: 1 if the reference kernels are selected
  */
 int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n);
+
+/*
+ * Stage timing (plans / batches created with SIE_FLAG_PROFILE; SIE_ESTATE otherwise).  Synchronises on the
+ * recorded events, sums the device time of every launch group enqueued since the last query, then clears.
+ *   ms[0..7):  0 coefficient transposes  1 unpack (packed -> square)  2 A1 GEMM  3 A2 GEMM  4 fused pair kernel
+ *              5 reduce/trace  6 reference kernels          (milliseconds, HOST array of n doubles)
+ *   ms[7..14): the number of launch groups summed into each of the seven entries above.
+ * sie_dfmp2_batch_timing reports the calling thread's last sie_dfmp2_batch call.
+ */
+int sie_dfmp2_plan_timing(sie_dfmp2_plan_t plan, double* ms, int n);
+int sie_dfmp2_batch_timing(double* ms, int n);
+
+/*
+ * FP64 issue-rate microkernels: the live denominator of the FP64 roofline.
+ *   kind 0: register-resident DMMA (mma.sync.m8n8k4.f64)   1: register-resident DFMA
+ *        2: shared-memory-fed DMMA with the fragment loads of the pair mainloop
+ *   iters: loop trips per warp;  ctas_per_sm: CTAs (256 threads) launched per SM;  scratch: >= 8 bytes, DEVICE.
+ * Runs the kernel twice on `cuda_stream`, times the second run with events, synchronises;
+ * *tflops (HOST) = flops / time, *ms (HOST, may be NULL) = that time.
+ */
+int sie_dfmp2_probe_fp64(int kind, int iters, int ctas_per_sm, void* scratch, double* tflops, double* ms, void* cuda_stream);
 
 #ifdef __cplusplus
 }

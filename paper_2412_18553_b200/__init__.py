@@ -5,6 +5,7 @@ this package is its thin Python binding.  Nothing here computes on the CPU and n
 """
 from .binding import (  # noqa: F401
     SIE_FLAG_HOST_IO,
+    SIE_FLAG_PROFILE,
     SIE_FLAG_REFERENCE,
     SIE_FLAG_VALIDATE,
     ClusterSolver,
@@ -17,5 +18,8 @@ from .binding import (  # noqa: F401
     sie_dfmp2_energy,
     sie_dfmp2_plan,
     sie_dfmp2_plan_info,
+    sie_dfmp2_plan_timing,
+    sie_dfmp2_batch_timing,
+    sie_dfmp2_probe_fp64,
     sie_dfmp2_transform,
 )

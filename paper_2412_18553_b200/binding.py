@@ -13,7 +13,7 @@ from typing import List, Optional, Sequence, Tuple
 import torch
 
 SIE_OK, SIE_EINVAL, SIE_ENOMEM, SIE_ECUDA, SIE_ESTATE, SIE_EGAP, SIE_EUNSUPPORTED = range(7)
-SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO = 1, 2, 4
+SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO, SIE_FLAG_PROFILE = 1, 2, 4, 8
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsie_dfmp2.so")
@@ -28,6 +28,9 @@ EXPORTS = (
     "sie_dfmp2_last_cuda_error",
     "sie_dfmp2_launch_count",
     "sie_dfmp2_plan_info",
+    "sie_dfmp2_plan_timing",
+    "sie_dfmp2_batch_timing",
+    "sie_dfmp2_probe_fp64",
 )
 
 
@@ -89,6 +92,13 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_launch_count.restype = ctypes.c_ulonglong
         L.sie_dfmp2_plan_info.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong), ci]
         L.sie_dfmp2_plan_info.restype = ci
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.sie_dfmp2_plan_timing.argtypes = [vp, dp, ci]
+        L.sie_dfmp2_plan_timing.restype = ci
+        L.sie_dfmp2_batch_timing.argtypes = [dp, ci]
+        L.sie_dfmp2_batch_timing.restype = ci
+        L.sie_dfmp2_probe_fp64.argtypes = [ci, ci, ci, vp, dp, dp, vp]
+        L.sie_dfmp2_probe_fp64.restype = ci
         _LIB = L
     return _LIB
 
@@ -158,6 +168,36 @@ def sie_dfmp2_plan_info(plan: int) -> dict:
     return {k: int(buf[i]) for i, k in enumerate(keys[:n])}
 
 
+STAGES = ("coeff_transpose", "unpack", "A1_gemm", "A2_gemm", "pair", "reduce", "reference")
+
+
+def _timing_dict(buf) -> dict:
+    n = len(STAGES)
+    return {"ms": {k: float(buf[i]) for i, k in enumerate(STAGES)}, "launch_groups": {k: int(buf[n + i]) for i, k in enumerate(STAGES)}}
+
+
+def sie_dfmp2_plan_timing(plan: int) -> dict:
+    """Per-stage device milliseconds since the last query (plan created with SIE_FLAG_PROFILE)."""
+    buf = (ctypes.c_double * (2 * len(STAGES)))()
+    _check(_lib().sie_dfmp2_plan_timing(plan, buf, len(buf)), "sie_dfmp2_plan_timing")
+    return _timing_dict(buf)
+
+
+def sie_dfmp2_batch_timing() -> dict:
+    buf = (ctypes.c_double * (2 * len(STAGES)))()
+    _check(_lib().sie_dfmp2_batch_timing(buf, len(buf)), "sie_dfmp2_batch_timing")
+    return _timing_dict(buf)
+
+
+def sie_dfmp2_probe_fp64(kind: int, iters: int = 20000, ctas_per_sm: int = 2, *, stream=None) -> Tuple[float, float]:
+    """-> (TFLOP/s, ms) of the FP64 issue-rate microkernel `kind` (0 DMMA, 1 DFMA, 2 smem-fed DMMA)."""
+    scratch = torch.zeros(8, dtype=torch.float64, device="cuda")
+    tf, ms = ctypes.c_double(), ctypes.c_double()
+    _check(_lib().sie_dfmp2_probe_fp64(kind, iters, ctas_per_sm, scratch.data_ptr(), ctypes.byref(tf), ctypes.byref(ms), _stream_ptr(stream)),
+           "sie_dfmp2_probe_fp64")
+    return tf.value, ms.value
+
+
 def _descs(clusters: Sequence[dict], host: bool) -> ctypes.Array:
     arr = (sie_dfmp2_cluster_t * max(1, len(clusters)))()
     for k, c in enumerate(clusters):
@@ -224,6 +264,9 @@ class ClusterSolver:
             E, G = E.pin_memory(), (G.pin_memory() if G is not None else None)
         sie_dfmp2_energy(self.plan, self.workspace, e_occ, e_vir, P_frag, E, G, host=self.host, stream=stream)
         return E, G
+
+    def timing(self) -> dict:
+        return sie_dfmp2_plan_timing(self.plan)
 
     def close(self) -> None:
         sie_dfmp2_destroy(self.plan)

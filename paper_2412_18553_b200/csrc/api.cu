@@ -110,8 +110,72 @@ static int check_device() {
 
 using namespace sie;
 
+// ------------------------------------------------------------------------------------------------ stage timing
+// SIE_FLAG_PROFILE: every launch group is bracketed by a pair of events on the caller's stream; the
+// elapsed times are summed per stage when queried (sie_dfmp2_plan_timing / sie_dfmp2_batch_timing).
+enum { ST_COEFF = 0, ST_UNPACK, ST_T1, ST_T2, ST_PAIR, ST_REDUCE, ST_REF, ST_COUNT };
+struct Prof {
+    bool on = false;
+    std::vector<cudaEvent_t> pool;
+    struct Span { int stage, e0, e1; };
+    std::vector<Span> spans;
+    size_t used = 0;
+    int take() {
+        if (used == pool.size()) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return -1;
+            pool.push_back(e);
+        }
+        return (int)used++;
+    }
+    int begin(int stage, cudaStream_t st) {
+        if (!on) return -1;
+        const int a = take(), b = take();
+        if (a < 0 || b < 0) return -1;
+        cudaEventRecord(pool[a], st);
+        spans.push_back(Span{stage, a, b});
+        return (int)spans.size() - 1;
+    }
+    void end(int span, cudaStream_t st) {
+        if (span >= 0) cudaEventRecord(pool[spans[span].e1], st);
+    }
+    void reset() {
+        spans.clear();
+        used = 0;
+    }
+    // sums per stage (ms) and launch-group counts; synchronises on the recorded events; then resets
+    int collect(double* ms, double* counts) {
+        for (int k = 0; k < ST_COUNT; ++k) ms[k] = counts[k] = 0.0;
+        for (const Span& s : spans) {
+            cudaError_t e = cudaEventSynchronize(pool[s.e1]);
+            float t = 0.f;
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&t, pool[s.e0], pool[s.e1]);
+            if (e != cudaSuccess) {
+                reset();
+                return set_cuda_error(e);
+            }
+            ms[s.stage] += t;
+            counts[s.stage] += 1.0;
+        }
+        reset();
+        return SIE_OK;
+    }
+    ~Prof() {
+        for (cudaEvent_t e : pool) cudaEventDestroy(e);
+    }
+};
+struct ProfSpan {  // RAII bracket
+    Prof& p;
+    cudaStream_t st;
+    int id;
+    ProfSpan(Prof& p_, int stage, cudaStream_t st_) : p(p_), st(st_), id(p_.begin(stage, st_)) {}
+    ~ProfSpan() { p.end(id, st); }
+};
+static thread_local Prof g_batch_prof;
+
 // ------------------------------------------------------------------------------------------------ plan
 struct sie_dfmp2_plan_s {
+    Prof prof;
     int nao = 0, o = 0, v = 0, naux = 0;
     unsigned flags = 0;
     bool ref = false;
@@ -164,7 +228,7 @@ void build_tiles(int nblk, std::vector<PairTile>& out) {
 int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags, bool carve_shared) {
     if (nao < 1 || nocc < 1 || nvir < 1 || naux < 1 || aux_block < 0) return SIE_EINVAL;
     if ((long long)nocc + nvir > nao) return SIE_EINVAL;
-    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO)) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE)) return SIE_EINVAL;
     p.nao = nao;
     p.o = nocc;
     p.v = nvir;
@@ -259,7 +323,7 @@ struct Scratch {  // shared transform scratch (device pointers)
 };
 
 // Transform of aux rows [p0,p1) into Bmat ([v][o][naux_ld]).  L points at row p0 (device, or host when host_L).
-int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, double* Bmat, const Scratch& sc, const double* dC_occ,
+int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof, double* Bmat, const Scratch& sc, const double* dC_occ,
                    const double* dC_vir, const double* L, bool host_L, int p0, int p1, cudaStream_t st) {
     const int nao = p.nao, o = p.o, v = p.v;
     if (p.ref) {
@@ -270,6 +334,7 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, double* Bm
                 SIE_CUDA(cudaMemcpyAsync(sc.stage, Lq, (size_t)(q1 - q0) * p.npair * 8, cudaMemcpyHostToDevice, st));
                 Lq = reinterpret_cast<const double*>(sc.stage);
             }
+            ProfSpan ps(prof, ST_REF, st);
             SIE_TRY(ref_transform(dC_occ, dC_vir, Lq, nao, o, v, q0, q1, sc.refH, Bmat, p.naux_ld, st));
         }
         return SIE_OK;
@@ -296,9 +361,13 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, double* Bm
             SIE_CUDA(cudaMemcpyAsync(dst, Lq, (size_t)pb * p.npair * 8, cudaMemcpyHostToDevice, po.copy_stream));
             SIE_CUDA(cudaEventRecord(po.ev_ready[buf], po.copy_stream));
             SIE_CUDA(cudaStreamWaitEvent(st, po.ev_ready[buf], 0));
-            SIE_TRY(launch_unpack(reinterpret_cast<const double*>(dst), pb, nao, sc.Lfull, p.nao_ld, st));
+            {
+                ProfSpan ps(prof, ST_UNPACK, st);
+                SIE_TRY(launch_unpack(reinterpret_cast<const double*>(dst), pb, nao, sc.Lfull, p.nao_ld, st));
+            }
             SIE_CUDA(cudaEventRecord(po.ev_consumed[buf], st));
         } else {
+            ProfSpan ps(prof, ST_UNPACK, st);
             SIE_TRY(launch_unpack(Lq, pb, nao, sc.Lfull, p.nao_ld, st));
         }
         // A1: H[i][P][nu] = sum_mu CoT[i][mu] * Lfull[P][nu][mu]
@@ -312,7 +381,10 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, double* Bm
         o1.valid_inner = nao;
         o1.stride_outer = p.nao_ld;
         o1.n_lin_total = (long long)pb * nvb * 128;
-        SIE_TRY(launch_gemm_tn(tm1, mapCo, mapL, 1, pb * nvb, nvb, (long long)nvb * 128, kblocks, o1, p.num_sms, st));
+        {
+            ProfSpan ps(prof, ST_T1, st);
+            SIE_TRY(launch_gemm_tn(tm1, mapCo, mapL, 1, pb * nvb, nvb, (long long)nvb * 128, kblocks, o1, p.num_sms, st));
+        }
         // A2: B[a][i][q0+P] = sum_nu CvT[a][nu] * H[(i,P)][nu]
         SIE_TRY(make_tensor_map_3d(&mapH, sc.H, nao, (uint64_t)o * pb, 1, (uint64_t)p.nao_ld * 8,
                                    (uint64_t)p.nao_ld * 8 * o * pb, 8, 128, 1));
@@ -325,13 +397,18 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, double* Bm
         o2.stride_outer = p.naux_ld;
         o2.n_lin_total = (long long)o * pb;
         const int m_tiles = (v + tm2 - 1) / tm2, n_tiles = (int)(((long long)o * pb + 127) / 128);
-        SIE_TRY(launch_gemm_tn(tm2, mapCv, mapH, m_tiles, n_tiles, n_tiles, 0, kblocks, o2, p.num_sms, st));
+        {
+            ProfSpan ps(prof, ST_T2, st);
+            SIE_TRY(launch_gemm_tn(tm2, mapCv, mapH, m_tiles, n_tiles, n_tiles, 0, kblocks, o2, p.num_sms, st));
+        }
     }
     return SIE_OK;
 }
 
-int prepare_coeffs(sie_dfmp2_plan_s& p, const Scratch& sc, const double* dC_occ, const double* dC_vir, cudaStream_t st) {
+int prepare_coeffs(sie_dfmp2_plan_s& p, Prof& prof, const Scratch& sc, const double* dC_occ, const double* dC_vir,
+                   cudaStream_t st) {
     if (p.ref) return SIE_OK;
+    ProfSpan ps(prof, ST_COEFF, st);
     SIE_TRY(launch_transpose(dC_occ, p.nao, p.o, sc.CoT, p.nao_ld, st));
     SIE_TRY(launch_transpose(dC_vir, p.nao, p.v, sc.CvT, p.nao_ld, st));
     return SIE_OK;
@@ -388,6 +465,7 @@ int sie_dfmp2_plan(sie_dfmp2_plan_t* plan, int nao, int nocc, int nvir, int naux
         delete p;
         return rc;
     }
+    p->prof.on = (flags & SIE_FLAG_PROFILE) != 0;
     *plan = p;
     *workspace_bytes = p->total;
     return SIE_OK;
@@ -422,12 +500,12 @@ int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_
             dCo = io + p.io_Cocc;
             dCv = io + p.io_Cvir;
         }
-        SIE_TRY(prepare_coeffs(p, sc, dCo, dCv, st));
+        SIE_TRY(prepare_coeffs(p, p.prof, sc, dCo, dCv, st));
         p.dC_occ = dCo;
         p.dC_vir = dCv;
         p.c_ready_ws = workspace;
     }
-    SIE_TRY(transform_rows(p, p, reinterpret_cast<double*>(ws + p.off_B), sc, p.dC_occ, p.dC_vir, L_packed_block, host, p0, p1, st));
+    SIE_TRY(transform_rows(p, p, p.prof, reinterpret_cast<double*>(ws + p.off_B), sc, p.dC_occ, p.dC_vir, L_packed_block, host, p0, p1, st));
     add_interval(p.covered, p0, p1);
     p.covered_rows += p1 - p0;
     return SIE_OK;
@@ -475,7 +553,10 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
     rc.o = o;
     if (p.ref) {
         double* G = reinterpret_cast<double*>(ws + p.off_refG);
-        SIE_TRY(ref_pair(Bmat, o, v, p.naux, p.naux_ld, de_occ, de_vir, reinterpret_cast<double*>(ws + p.off_refVj), G, st));
+        {
+            ProfSpan ps(p.prof, ST_REF, st);
+            SIE_TRY(ref_pair(Bmat, o, v, p.naux, p.naux_ld, de_occ, de_vir, reinterpret_cast<double*>(ws + p.off_refVj), G, st));
+        }
         rc.gpart = G;
         rc.o8 = o;
         rc.nslots = 1;
@@ -486,14 +567,20 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
         SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
         SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
         SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)p.ncta * p.kp * p.o8 * p.o8 * 8, st));
-        SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc), reinterpret_cast<const PairTile*>(ws + p.off_tiles),
-                            (int)p.tiles.size(), p.ncta, st));
+        {
+            ProfSpan ps(p.prof, ST_PAIR, st);
+            SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc),
+                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, st));
+        }
         rc.gpart = gpart;
         rc.o8 = p.o8;
         rc.nslots = p.ncta * p.kp;
     }
     SIE_CUDA(cudaMemcpyAsync(ws + p.off_rc, &rc, sizeof rc, cudaMemcpyHostToDevice, st));
-    SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
+    {
+        ProfSpan ps(p.prof, ST_REDUCE, st);
+        SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
+    }
     if (host) {
         SIE_CUDA(cudaMemcpyAsync(E_out, dE, 8, cudaMemcpyDeviceToHost, st));
         if (G_out) SIE_CUDA(cudaMemcpyAsync(G_out, dG, (size_t)o * o * 8, cudaMemcpyDeviceToHost, st));
@@ -505,10 +592,14 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
 int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes, size_t* needed,
                     unsigned flags, void* cuda_stream) {
     if (ncluster < 0 || (ncluster > 0 && !clusters)) return SIE_EINVAL;
-    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO)) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE)) return SIE_EINVAL;
     const bool host = flags & SIE_FLAG_HOST_IO;
     const bool query = (workspace == nullptr || workspace_bytes == 0);
     if (query && !needed) return SIE_EINVAL;
+    if (ncluster == 0) {  // nothing to schedule: no workspace, no launch
+        if (needed) *needed = 0;
+        return SIE_OK;
+    }
     try {
         // ---- per-cluster plans (B + partial-G regions) and shared scratch sized for the largest cluster
         std::vector<sie_dfmp2_plan_s> plans(ncluster);
@@ -519,7 +610,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             const sie_dfmp2_cluster_t& cl = clusters[k];
             if (!query && (!cl.C_occ || !cl.C_vir || !cl.L_packed || !cl.e_occ || !cl.e_vir || !cl.E_out)) return SIE_EINVAL;
             sie_dfmp2_plan_s& p = plans[k];
-            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~SIE_FLAG_HOST_IO, false));
+            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~(SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE), false));
             off_cl[k] = c.take(p.total);
             if (!p.ref) {
                 max_CoT = std::max(max_CoT, (size_t)p.o * p.nao_ld * 8);
@@ -553,6 +644,9 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
 
         cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
         unsigned char* ws = static_cast<unsigned char*>(workspace);
+        Prof& prof = g_batch_prof;
+        prof.reset();
+        prof.on = (flags & SIE_FLAG_PROFILE) != 0;
         sie_dfmp2_plan_s pipe;  // owns the HOST_IO copy stream/events of this call
         struct PipeGuard {
             sie_dfmp2_plan_s& p;
@@ -618,8 +712,8 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                 SIE_CUDA(cudaStreamSynchronize(st));
                 SIE_TRY(check_gap_host(he.data(), he.data() + p.o, p.o, p.v));
             }
-            SIE_TRY(prepare_coeffs(p, sc, dCo, dCv, st));
-            SIE_TRY(transform_rows(p, pipe, reinterpret_cast<double*>(wk + p.off_B), sc, dCo, dCv, cl.L_packed, host, 0, p.naux, st));
+            SIE_TRY(prepare_coeffs(p, prof, sc, dCo, dCv, st));
+            SIE_TRY(transform_rows(p, pipe, prof, reinterpret_cast<double*>(wk + p.off_B), sc, dCo, dCv, cl.L_packed, host, 0, p.naux, st));
             rcs[k] = ReduceCluster{};
             rcs[k].P = dP;
             rcs[k].E_out = dE[k];
@@ -651,6 +745,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         if (!tiles.empty()) {
             SIE_CUDA(cudaMemcpyAsync(ws + off_desc, descs.data(), descs.size() * sizeof(PairCluster), cudaMemcpyHostToDevice, st));
             SIE_CUDA(cudaMemcpyAsync(ws + off_tiles, tiles.data(), tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+            ProfSpan ps(prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
                                 (int)tiles.size(), ncta, st));
         }
@@ -660,14 +755,20 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             if (!p.ref) continue;
             unsigned char* wk = ws + off_cl[k];
             double* G = reinterpret_cast<double*>(wk + p.off_refG);
-            SIE_TRY(ref_pair(reinterpret_cast<const double*>(wk + p.off_B), p.o, p.v, p.naux, p.naux_ld, de_occ[k], de_vir[k],
-                             reinterpret_cast<double*>(ws + off_refVj), G, st));
+            {
+                ProfSpan ps(prof, ST_REF, st);
+                SIE_TRY(ref_pair(reinterpret_cast<const double*>(wk + p.off_B), p.o, p.v, p.naux, p.naux_ld, de_occ[k], de_vir[k],
+                                 reinterpret_cast<double*>(ws + off_refVj), G, st));
+            }
             rcs[k].gpart = G;
             rcs[k].o8 = p.o;
             rcs[k].nslots = 1;
         }
         SIE_CUDA(cudaMemcpyAsync(ws + off_rc, rcs.data(), rcs.size() * sizeof(ReduceCluster), cudaMemcpyHostToDevice, st));
-        SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + off_rc), ncluster, st));
+        {
+            ProfSpan ps(prof, ST_REDUCE, st);
+            SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + off_rc), ncluster, st));
+        }
         if (host) {
             for (int k = 0; k < ncluster; ++k) {
                 SIE_CUDA(cudaMemcpyAsync(clusters[k].E_out, dE[k], 8, cudaMemcpyDeviceToHost, st));
@@ -713,6 +814,38 @@ const char* sie_dfmp2_strerror(int status) {
 const char* sie_dfmp2_last_cuda_error(void) { return g_last_error.c_str(); }
 
 unsigned long long sie_dfmp2_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+static int timing_out(Prof& prof, double* ms, int n) {
+    double t[ST_COUNT], c[ST_COUNT];
+    SIE_TRY(prof.collect(t, c));
+    for (int k = 0; k < n && k < 2 * ST_COUNT; ++k)
+        if (ms) ms[k] = k < ST_COUNT ? t[k] : c[k - ST_COUNT];
+    return SIE_OK;
+}
+
+int sie_dfmp2_plan_timing(sie_dfmp2_plan_t plan, double* ms, int n) {
+    if (!plan || !ms || n < 0) return SIE_EINVAL;
+    if (!plan->prof.on) return SIE_ESTATE;
+    return timing_out(plan->prof, ms, n);
+}
+
+int sie_dfmp2_batch_timing(double* ms, int n) {
+    if (!ms || n < 0) return SIE_EINVAL;
+    if (!g_batch_prof.on) return SIE_ESTATE;
+    return timing_out(g_batch_prof, ms, n);
+}
+
+int sie_dfmp2_probe_fp64(int kind, int iters, int ctas_per_sm, void* scratch, double* tflops, double* ms, void* cuda_stream) {
+    if (!scratch || !tflops) return SIE_EINVAL;
+    SIE_TRY(check_device());
+    double flops = 0.0;
+    float t = 0.f;
+    SIE_TRY(run_probe(kind, iters, ctas_per_sm, query_num_sms(), static_cast<double*>(scratch), &flops, &t,
+                      static_cast<cudaStream_t>(cuda_stream)));
+    *tflops = flops / (t * 1e-3) * 1e-12;
+    if (ms) *ms = t;
+    return SIE_OK;
+}
 
 int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n) {
     if (!plan) return 0;

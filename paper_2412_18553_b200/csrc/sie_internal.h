@@ -71,4 +71,7 @@ int ref_pair(const double* B, int o, int v, int naux, int naux_ld, const double*
              double* Vj /*[o][v][v]*/, double* G /*[o][o]*/, cudaStream_t st);
 size_t ref_vj_bytes(int o, int v);
 
+// ---- probes.cu ---------------------------------------------------------------------------------
+int run_probe(int kind, int iters, int ctas_per_sm, int num_sms, double* sink, double* flops, float* ms, cudaStream_t st);
+
 }  // namespace sie

@@ -22,7 +22,7 @@ def _built():
 def _declared_symbols():
     text = open(os.path.join(ROOT, "include", "sie_dfmp2.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(sie_dfmp2_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(sie_dfmp2_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_library_exports_every_declared_symbol():
