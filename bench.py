@@ -9,6 +9,7 @@ projector/trace reduction) over one synthetic workload of BASELINE.json:
     config1                          one cluster o=30 v=270 nao=300 naux=1200
     config2                          96 clusters through sie_dfmp2_batch (clusters/s)
     config4:<k>                      sweep point k in 0..3 (o=64, v=256/512/1024/2048)
+    custom:o,v,naux                  one cluster of that shape (nao=o+v): short slices for ncu captures
 `value` is algorithmic FP64 TFLOP/s (minimum flops of the method / device time) with the inputs resident in HBM;
 `e2e` is the same metric through the C ABI with HOST (pinned) buffers, H2D/D2H inside the timed region.
 N > 1 (torchrun): independent replicas, one cluster (batch) per GPU, no data-path collective ("replicas only").
@@ -56,18 +57,22 @@ def alg_flops(s: ClusterSpec) -> dict:
 
 
 def exec_pair_flops(s: ClusterSpec, info: dict) -> float:
-    """Flops the pair kernel issues on the tensor pipe: padded 128x128 SYRK tiles over ceil(naux/8) K-blocks,
-    plus the G update (two DMMA passes per off-diagonal virtual pair, one per diagonal pair)."""
+    """Flops the pair kernel issues on the tensor pipe: TM x TN SYRK tiles (TM = ceil8(ta*nocc)) over ceil(naux/8)
+    K-blocks, plus the G update (two DMMA passes of ceil8(o) x ceil8(o) x ceil4(o) per unordered virtual pair)."""
     kblocks = (s.naux + 7) // 8
     main = 2.0 * info["TM"] * info["TN"] * 8 * kblocks * info["ntiles"]
     o8, v = info["o8"], s.nvir
-    epi = 2.0 * o8 ** 3 * (v * (v - 1) + v)
+    o4 = (s.nocc + 3) // 4 * 4
+    epi = 2.0 * o8 * o8 * o4 * (v * (v + 1))
     return main + epi
 
 
 def workload_specs(name: str, rank: int):
     """Cluster list of one replica. Replica r > 0 draws its own clusters (cluster_id shifted by 1000 r)."""
-    if name.startswith("config4"):
+    if name.startswith("custom:"):  # profiling slices, e.g. custom:120,216,4800 = a 1/5-virtuals slice of config 3
+        o, v, naux = (int(x) for x in name.split(":")[1].split(",")[:3])
+        specs = [ClusterSpec(9, 0, o + v, o, v, naux, max(1, o // 2))]
+    elif name.startswith("config4"):
         k = int(name.split(":")[1]) if ":" in name else 2
         specs = [config_specs(4)[2 * k]]
     else:

@@ -123,8 +123,8 @@ unsigned long long sie_dfmp2_launch_count(void);
 
 /*
  * Introspection for benchmarks/tests: fills info[0..n) with plan facts, returns how many exist.
- *   0: pair-tile rows TM   1: pair-tile cols TN   2: virtual sub-blocks per tile side (ta)
- *   3: nocc padded to 8 (o8)   4: number of pair tiles   5: persistent CTAs   6: internal aux sub-block
+ *   0, 1: pair-tile rows / cols in rows of B, ceil8(ta*nocc) <= 128   2: virtual blocks per tile side (ta)
+ *   3: ceil8(nocc), the leading dimension of a partial-G slot   4: number of pair tiles   5: persistent CTAs   6: internal aux sub-block
  *   7: 1 if the reference kernels are selected
  */
 int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n);

@@ -179,7 +179,7 @@ struct sie_dfmp2_plan_s {
     int nao = 0, o = 0, v = 0, naux = 0;
     unsigned flags = 0;
     bool ref = false;
-    int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, nblk = 0, pblk = 0, ncta = 0, kp = 1, num_sms = 148;
+    int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, t8 = 8, nblk = 0, pblk = 0, ncta = 0, kp = 1, num_sms = 148;
     size_t npair = 0;
     std::vector<PairTile> tiles;  // cluster field = 0; rewritten when used inside a batch
     double tile_cost = 0;         // relative cost of one tile (for batch ordering)
@@ -256,15 +256,17 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
         p.pblk = std::min(pb, naux);
     }
     if (!p.ref) {
-        if (nvir > 65535 * (geo.TM / p.o8 > 0 ? geo.TM / p.o8 : 1)) return SIE_EINVAL;
-        p.ta = std::max(1, geo.TM / p.o8);
+        // pair tiling: ta whole virtual blocks (ta*o <= 128 rows of B, o itself is never padded) per tile edge
+        p.ta = std::max(1, geo.TM / nocc);
+        p.t8 = (int)align_up((size_t)p.ta * nocc, 8);
         p.nblk = (nvir + p.ta - 1) / p.ta;
+        if (p.nblk > 65535) return SIE_EINVAL;
         build_tiles(p.nblk, p.tiles);
         p.ncta = (int)std::min<size_t>((size_t)p.num_sms, p.tiles.size());
-        const int nt8 = p.o8 / 8;
-        p.kp = nt8 >= geo.ncons ? 1 : geo.ncons / nt8;
+        const int nst = p.o8 / 8;
+        p.kp = nst >= geo.ncons ? 1 : geo.ncons / nst;
         p.gpart_bytes = (size_t)p.num_sms * p.kp * p.o8 * p.o8 * 8;  // sized for any CTA count up to num_sms
-        p.tile_cost = (double)geo.TM * geo.TN * naux + 4.0 * p.ta * p.ta * (double)p.o8 * p.o8 * p.o8;
+        p.tile_cost = (double)p.t8 * p.t8 * naux + 4.0 * p.ta * p.ta * (double)p.o8 * p.o8 * p.o8;
     }
     // workspace
     Carver c;
@@ -417,7 +419,8 @@ int prepare_coeffs(sie_dfmp2_plan_s& p, Prof& prof, const Scratch& sc, const dou
 int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const double* de_occ, const double* de_vir, double* gpart,
                       int kp, PairCluster& d) {
     std::memset(&d, 0, sizeof d);
-    SIE_TRY(make_tensor_map_3d(&d.map, Bmat, p.naux, p.o, p.v, (uint64_t)p.naux_ld * 8, (uint64_t)p.o * p.naux_ld * 8, 8, p.o8, p.ta));
+    const uint64_t rows = (uint64_t)p.o * p.v;  // B[a][i][P] read as a plain (v*o) x naux matrix, row = a*o + i
+    SIE_TRY(make_tensor_map_3d(&d.map, Bmat, p.naux, rows, 1, (uint64_t)p.naux_ld * 8, rows * p.naux_ld * 8, 8, p.t8, 1));
     d.e_occ = de_occ;
     d.e_vir = de_vir;
     d.gpart = gpart;
@@ -427,7 +430,8 @@ int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const doubl
     d.ta = p.ta;
     d.kblocks = (p.naux + 7) / 8;
     d.kp = kp;
-    d.tx_bytes = 2u * 8u * (uint32_t)p.o8 * (uint32_t)p.ta * 8u;
+    d.t8 = p.t8;
+    d.tx_bytes = 2u * 8u * (uint32_t)p.t8 * 8u;
     return SIE_OK;
 }
 
@@ -570,7 +574,7 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
         {
             ProfSpan ps(p.prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc),
-                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, st));
+                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8, st));
         }
         rc.gpart = gpart;
         rc.o8 = p.o8;
@@ -728,6 +732,8 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         const int ncta = (int)std::min<size_t>((size_t)plans[0].num_sms, std::max<size_t>(1, ntiles_total));
         std::vector<PairTile> tiles;
         tiles.reserve(ntiles_total);
+        int tmax = 8;
+        for (int k : order) tmax = std::max(tmax, plans[k].t8);
         for (int k : order) {
             sie_dfmp2_plan_s& p = plans[k];
             unsigned char* wk = ws + off_cl[k];
@@ -747,7 +753,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_CUDA(cudaMemcpyAsync(ws + off_tiles, tiles.data(), tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
             ProfSpan ps(prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
-                                (int)tiles.size(), ncta, st));
+                                (int)tiles.size(), ncta, tmax, st));
         }
         // reference-path clusters (nocc > 128 or SIE_FLAG_REFERENCE): per-j kernels, one cluster at a time
         for (int k = 0; k < ncluster; ++k) {
@@ -850,7 +856,7 @@ int sie_dfmp2_probe_fp64(int kind, int iters, int ctas_per_sm, void* scratch, do
 int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n) {
     if (!plan) return 0;
     const PairGeom geo = pair_geom();
-    const long long vals[8] = {geo.TM, geo.TN, plan->ta, plan->o8, (long long)plan->tiles.size(), plan->ncta, plan->pblk, plan->ref ? 1 : 0};
+    const long long vals[8] = {plan->t8, plan->t8, plan->ta, plan->o8, (long long)plan->tiles.size(), plan->ncta, plan->pblk, plan->ref ? 1 : 0};
     for (int i = 0; i < n && i < 8; ++i)
         if (info) info[i] = vals[i];
     return 8;

@@ -24,6 +24,12 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 
+__device__ __forceinline__ double2 lds128(uint32_t addr) {  // 16-byte shared load from a 32-bit shared address
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+
 // ------------------------------------------------------------------------------------------------
 // mbarrier (shared::cta, 64-bit)
 // ------------------------------------------------------------------------------------------------

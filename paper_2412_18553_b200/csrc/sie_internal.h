@@ -33,15 +33,15 @@ int gemm_tm_for(int m);  // smallest supported M-tile height covering min(m,128)
 
 // ---- pair.cu -----------------------------------------------------------------------------------
 struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (global memory)
-    CUtensorMap map;               // B as {naux, nocc, nvir}, box {8, o8, ta}
+    CUtensorMap map;               // B as the plain matrix {naux, nocc*nvir, 1}, box {8, t8, 1}
     const double* e_occ;
     const double* e_vir;
     double* gpart;                 // partial-G slots of this cluster: [ncta][kp][o8*o8]
-    int o, v, o8, ta;
+    int o, v, o8, ta;              // o8 = ceil8(o): leading dimension of a partial-G slot; ta virtual blocks per tile edge
     int kblocks;                   // ceil(naux / 8)
-    int kp;                        // epilogue K-split parts
+    int kp;                        // epilogue sub-block split parts
     uint32_t tx_bytes;             // bytes of both operand boxes of one stage
-    int pad_;
+    int t8;                        // tile edge in rows of B: ceil8(ta * o) <= 128
 };
 struct PairTile {                  // 8 bytes
     int cluster;
@@ -52,7 +52,7 @@ struct PairGeom {                  // tile configuration facts for host-side pla
 };
 PairGeom pair_geom();
 size_t pair_smem_bytes();
-int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, cudaStream_t st);
+int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, cudaStream_t st);
 
 struct ReduceCluster {             // per cluster, device array
     const double* gpart;           // [nslots][o8*o8]

@@ -45,7 +45,7 @@ def test_library_does_not_link_libcuda():
 def test_plan_is_host_only_and_reports_workspace():
     plan, ws = sie.sie_dfmp2_plan(48, 8, 40, 160)
     info = sie.sie_dfmp2_plan_info(plan)
-    assert info["TM"] == 128 and info["TN"] == 128 and info["o8"] == 8 and info["ta"] == 16
+    assert info["TM"] == 128 and info["TN"] == 128 and info["o8"] == 8 and info["ta"] == 16  # 16 blocks of o=8 rows
     nblk = (40 + 15) // 16
     assert info["ntiles"] == nblk * (nblk + 1) // 2 and info["reference"] == 0
     assert ws >= 40 * 8 * 160 * 8  # at least B
@@ -53,9 +53,15 @@ def test_plan_is_host_only_and_reports_workspace():
     # config 3: B alone is ~5 GB; 1080 virtual blocks -> 584k tiles
     plan, ws = sie.sie_dfmp2_plan(1200, 120, 1080, 4800)
     info = sie.sie_dfmp2_plan_info(plan)
-    assert info["ta"] == 1 and info["o8"] == 120 and info["ntiles"] == 1080 * 1081 // 2 and info["ncta"] == 148
+    assert info["TM"] == 120 and info["ta"] == 1 and info["o8"] == 120 and info["ntiles"] == 1080 * 1081 // 2 and info["ncta"] == 148
     assert 4.9e9 < ws < 7e9
     sie.sie_dfmp2_destroy(plan)
+    # o is never padded inside a tile: o=30 -> 4 blocks = 120 rows exactly; o=17 -> 7 blocks = 119 rows -> 120
+    for o, ta, t8 in ((30, 4, 120), (17, 7, 120), (33, 3, 104), (65, 1, 72), (128, 1, 128)):
+        plan, _ = sie.sie_dfmp2_plan(10 * o, o, 8 * o, 100)
+        info = sie.sie_dfmp2_plan_info(plan)
+        assert (info["ta"], info["TM"], info["TN"]) == (ta, t8, t8), (o, info)
+        sie.sie_dfmp2_destroy(plan)
     # nocc > 128 -> reference kernels
     plan, _ = sie.sie_dfmp2_plan(400, 130, 200, 300)
     assert sie.sie_dfmp2_plan_info(plan)["reference"] == 1
