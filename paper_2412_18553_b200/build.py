@@ -35,7 +35,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, *( ["-Xptxas", "-v"] if verbose else []), "-o", LIB, *[os.path.join(CSRC, f) for f in SOURCES]]
+    extra = os.environ.get("SIE_NVCC_EXTRA", "").split()  # e.g. -DSIE_EXP_...=1 for kernel experiments
+    cmd = [nvcc, *NVCC_FLAGS, *extra, *( ["-Xptxas", "-v"] if verbose else []), "-o", LIB, *[os.path.join(CSRC, f) for f in SOURCES]]
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -247,10 +247,12 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
     } else if (p.ref) {
         p.pblk = std::min(naux, 64);
     } else {
+        // aux sub-block: enough 128-column tiles of A1 for ~8 full waves of the persistent GEMM (tail < 1/8 wave),
+        // at most 128 aux rows and at most 2 GB for the unpacked square block
         const int nvb = (nao + 127) / 128;
-        int pb = (2 * p.num_sms + nvb - 1) / nvb;
+        int pb = (8 * p.num_sms + nvb - 1) / nvb;
         const size_t per_p = (size_t)nao * p.nao_ld * 8;
-        const int cap = (int)std::max<size_t>(8, ((size_t)512 << 20) / per_p);
+        const int cap = (int)std::max<size_t>(8, ((size_t)2048 << 20) / per_p);
         pb = std::max(8, std::min(std::min(pb, 128), cap));
         pb = (pb + 7) / 8 * 8;
         p.pblk = std::min(pb, naux);
