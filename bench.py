@@ -38,7 +38,10 @@ METRIC = "DF-MP2 cluster energy: FP64 TFLOP/s (algorithmic) & % of FP64 peak; cl
 UNIT = "TFLOP/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pair_kernel launch, from the committed ncu --set full
 # captures under profiles/ (file named beside each number); None = not captured for that workload.
-NCU_PAIR_TRAFFIC_BYTES = {}
+NCU_PAIR_TRAFFIC_BYTES = {
+    "config3": 524.166e9 + 87.257e9,              # profiles/r01_ncu_pair_rev2_config3.md
+    "custom:120,216,4800": 21.139e9 + 3.481e9,    # profiles/r01_ncu_pair_rev2_slice.md
+}
 
 
 # ------------------------------------------------------------------------------------------------ flop model
@@ -136,7 +139,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ CPU oracle arm
-def oracle_sample(spec: ClusterSpec, n_aux_rows: int = 32, n_j: int = 8, v_sub: int = 192, seed: int = 7):
+def oracle_sample(spec: ClusterSpec, n_aux_rows: int = 96, n_j: int = 16, v_sub: int = 256, seed: int = 7):
     """Time the oracle (oracle/dfmp2_oracle.c, as it stands) on a bounded sample of `spec` and extrapolate.
 
     Sample: (a) O1-O3 for the first `n_aux_rows` aux rows at the full nao/nocc/nvir; (b) O4-O7 for j in [0, n_j),
@@ -178,7 +181,7 @@ def oracle_workload_seconds(specs, budget_per_cluster=None):
     if small:  # tiny cluster: run all of it
         n_rows, n_j, v_sub = big.naux, big.nocc, big.nvir
     else:
-        n_rows, n_j, v_sub = 32, 8, min(big.nvir, 192)  # ~10-20 s of CPU work on 16 cores at config 3
+        n_rows, n_j, v_sub = 96, 16, min(big.nvir, 256)  # ~15 s of CPU work on 16 cores at config 3
     tot, spent, desc = oracle_sample(big, n_rows, n_j, v_sub)
     rate = alg_flops(big)["total"] / tot  # algorithmic flop/s of the oracle
     secs = sum(alg_flops(s)["total"] for s in specs) / rate
