@@ -284,7 +284,7 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
             p.off_Lfull = c.take((size_t)p.pblk * nao * p.nao_ld * 8);
             p.off_H = c.take((size_t)nocc * p.pblk * p.nao_ld * 8);
             p.off_desc = c.take(sizeof(PairCluster));
-            p.off_tiles = c.take(p.tiles.size() * sizeof(PairTile));
+            p.off_tiles = c.take(p.tiles.size() * sizeof(PairTile) + 256);  // + the round-gate counter behind the list
         } else {
             p.off_refH = c.take((size_t)p.pblk * nocc * nao * 8);
             p.off_refVj = c.take(ref_vj_bytes(nocc, nvir));
@@ -437,6 +437,41 @@ int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const doubl
     return SIE_OK;
 }
 
+constexpr int BATCH_LANES = 4;
+
+// side streams of one batch call: forked from / joined into the caller's stream with events
+struct LaneStreams {
+    std::vector<cudaStream_t> streams;
+    std::vector<cudaEvent_t> done;
+    cudaEvent_t start = nullptr;
+    int fork(int n, cudaStream_t st) {
+        SIE_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+        SIE_CUDA(cudaEventRecord(start, st));
+        for (int l = 0; l < n; ++l) {
+            cudaStream_t s;
+            cudaEvent_t e;
+            SIE_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+            streams.push_back(s);
+            SIE_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            done.push_back(e);
+            SIE_CUDA(cudaStreamWaitEvent(s, start, 0));
+        }
+        return SIE_OK;
+    }
+    int join(cudaStream_t st) {
+        for (size_t l = 0; l < streams.size(); ++l) {
+            SIE_CUDA(cudaEventRecord(done[l], streams[l]));
+            SIE_CUDA(cudaStreamWaitEvent(st, done[l], 0));
+        }
+        return SIE_OK;
+    }
+    ~LaneStreams() {  // destruction is deferred by the runtime until the enqueued work has completed
+        for (cudaEvent_t e : done) cudaEventDestroy(e);
+        if (start) cudaEventDestroy(start);
+        for (cudaStream_t s : streams) cudaStreamDestroy(s);
+    }
+};
+
 int check_gap_host(const double* e_occ, const double* e_vir, int o, int v) {
     double mo = e_occ[0], mv = e_vir[0];
     for (int i = 1; i < o; ++i) mo = std::max(mo, e_occ[i]);
@@ -570,8 +605,10 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
         double* gpart = reinterpret_cast<double*>(ws + p.off_gpart);
         PairCluster pc;
         SIE_TRY(fill_pair_cluster(p, Bmat, de_occ, de_vir, gpart, p.kp, pc));
+        pc.gate = 1;  // one cluster: all tiles cost the same, keep the CTAs in K-lockstep for L2
         SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
         SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+        SIE_CUDA(cudaMemsetAsync(ws + p.off_tiles + p.tiles.size() * sizeof(PairTile), 0, 256, st));
         SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)p.ncta * p.kp * p.o8 * p.o8 * 8, st));
         {
             ProfSpan ps(p.prof, ST_PAIR, st);
@@ -634,11 +671,16 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                 off_io[k] = c.take(d * 8);
             }
         }
-        const size_t off_CoT = c.take(max_CoT), off_CvT = c.take(max_CvT), off_Lfull = c.take(max_Lfull), off_H = c.take(max_H);
-        const size_t off_refH = c.take(max_refH), off_refVj = c.take(max_refVj);
+        // transform lanes: the per-cluster transforms of a batch are many small launches (config 2: ~2900), so they are
+        // dealt to a few side streams with private scratch and run concurrently; the pair launch joins them
+        const int nlanes = (host || (flags & SIE_FLAG_VALIDATE)) ? 1 : std::min(BATCH_LANES, ncluster);
+        const size_t lane_bytes = align_up(max_CoT, 256) + align_up(max_CvT, 256) + align_up(max_Lfull, 256) + align_up(max_H, 256) +
+                                  align_up(max_refH, 256);
+        const size_t off_lanes = c.take(lane_bytes * nlanes);
+        const size_t off_refVj = c.take(max_refVj);
         const size_t off_stage = host ? c.take(2 * max_stage) : 0;
         const size_t off_desc = c.take((size_t)std::max(1, ncluster) * sizeof(PairCluster));
-        const size_t off_tiles = c.take(std::max<size_t>(1, ntiles_total) * sizeof(PairTile));
+        const size_t off_tiles = c.take(std::max<size_t>(1, ntiles_total) * sizeof(PairTile) + 256);
         const size_t off_rc = c.take((size_t)std::max(1, ncluster) * sizeof(ReduceCluster));
         const size_t total = c.off;
         if (needed) *needed = total;
@@ -670,14 +712,20 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             }
         } guard{pipe};
 
-        Scratch sc{};
-        sc.CoT = reinterpret_cast<double*>(ws + off_CoT);
-        sc.CvT = reinterpret_cast<double*>(ws + off_CvT);
-        sc.Lfull = reinterpret_cast<double*>(ws + off_Lfull);
-        sc.H = reinterpret_cast<double*>(ws + off_H);
-        sc.refH = reinterpret_cast<double*>(ws + off_refH);
-        sc.stage = ws + off_stage;
-        sc.stage_buf_bytes = max_stage;
+        std::vector<Scratch> lanes(nlanes);
+        for (int l = 0; l < nlanes; ++l) {
+            unsigned char* b = ws + off_lanes + (size_t)l * lane_bytes;
+            Scratch& sc = lanes[l];
+            sc.CoT = reinterpret_cast<double*>(b), b += align_up(max_CoT, 256);
+            sc.CvT = reinterpret_cast<double*>(b), b += align_up(max_CvT, 256);
+            sc.Lfull = reinterpret_cast<double*>(b), b += align_up(max_Lfull, 256);
+            sc.H = reinterpret_cast<double*>(b), b += align_up(max_H, 256);
+            sc.refH = reinterpret_cast<double*>(b);
+            sc.stage = ws + off_stage;
+            sc.stage_buf_bytes = max_stage;
+        }
+        LaneStreams ls;
+        if (nlanes > 1) SIE_TRY(ls.fork(nlanes, st));
 
         std::vector<PairCluster> descs(ncluster);
         std::vector<ReduceCluster> rcs(ncluster);
@@ -718,14 +766,18 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                 SIE_CUDA(cudaStreamSynchronize(st));
                 SIE_TRY(check_gap_host(he.data(), he.data() + p.o, p.o, p.v));
             }
-            SIE_TRY(prepare_coeffs(p, prof, sc, dCo, dCv, st));
-            SIE_TRY(transform_rows(p, pipe, prof, reinterpret_cast<double*>(wk + p.off_B), sc, dCo, dCv, cl.L_packed, host, 0, p.naux, st));
+            const int lane = k % nlanes;
+            cudaStream_t sk = nlanes > 1 ? ls.streams[lane] : st;
+            SIE_TRY(prepare_coeffs(p, prof, lanes[lane], dCo, dCv, sk));
+            SIE_TRY(transform_rows(p, pipe, prof, reinterpret_cast<double*>(wk + p.off_B), lanes[lane], dCo, dCv, cl.L_packed, host, 0,
+                                   p.naux, sk));
             rcs[k] = ReduceCluster{};
             rcs[k].P = dP;
             rcs[k].E_out = dE[k];
             rcs[k].G_out = dG[k];
             rcs[k].o = p.o;
         }
+        if (nlanes > 1) SIE_TRY(ls.join(st));
         // ---- stage 2: one persistent pair launch over all (cluster, tile) items, most expensive tiles first
         std::vector<int> order;
         for (int k = 0; k < ncluster; ++k)
@@ -753,6 +805,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         if (!tiles.empty()) {
             SIE_CUDA(cudaMemcpyAsync(ws + off_desc, descs.data(), descs.size() * sizeof(PairCluster), cudaMemcpyHostToDevice, st));
             SIE_CUDA(cudaMemcpyAsync(ws + off_tiles, tiles.data(), tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+            SIE_CUDA(cudaMemsetAsync(ws + off_tiles + tiles.size() * sizeof(PairTile), 0, 256, st));
             ProfSpan ps(prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
                                 (int)tiles.size(), ncta, tmax, st));

@@ -42,6 +42,7 @@ struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (g
     int kp;                        // epilogue sub-block split parts
     uint32_t tx_bytes;             // bytes of both operand boxes of one stage
     int t8;                        // tile edge in rows of B: ceil8(ta * o) <= 128
+    int gate;                      // 1: producers keep the CTAs of a round in K-lockstep (equal-cost tiles only)
 };
 struct PairTile {                  // 8 bytes
     int cluster;
