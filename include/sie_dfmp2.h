@@ -93,6 +93,11 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
  *    static, cost-balanced list of (cluster, tile) work items, then one reduction launch (step A7).
  *      clusters: HOST array of descriptors (pointers device or host per SIE_FLAG_HOST_IO).
  *      workspace_bytes == 0 or workspace == NULL: query only, *needed receives the required size.
+ *    With device pointers the per-cluster transforms run on up to 4 internal side streams that are forked from
+ *    and joined back into `cuda_stream` with events (all work is ordered after what was enqueued on `cuda_stream`
+ *    before the call, and the results are ready when `cuda_stream` reaches the end of the call's work).
+ *    Errors: SIE_EINVAL (sizes, null required pointers, misaligned workspace), SIE_ENOMEM (workspace too small;
+ *    *needed is set), SIE_EGAP (SIE_FLAG_VALIDATE), SIE_ECUDA.  Outputs are untouched on SIE_EINVAL/SIE_ENOMEM.
  */
 typedef struct {
     int nao, nocc, nvir, naux;
