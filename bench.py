@@ -39,8 +39,7 @@ UNIT = "TFLOP/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE pair_kernel launch, from the committed ncu --set full
 # captures under profiles/ (file named beside each number); None = not captured for that workload.
 NCU_PAIR_TRAFFIC_BYTES = {
-    "config3": 524.166e9 + 87.257e9,              # profiles/r01_ncu_pair_rev2_config3.md
-    "custom:120,216,4800": 21.139e9 + 3.481e9,    # profiles/r01_ncu_pair_rev2_slice.md
+    "config3": 529.222e9 + 85.369e9,              # profiles/r01_ncu_pair_rev3_config3.md
 }
 
 
