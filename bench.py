@@ -502,6 +502,7 @@ def run_streamed(args) -> None:
             x.L_block(p0, p1, out=pinned.numpy()[: p1 - p0], threads=ncpu)
             torch.cuda.synchronize()  # the previous transform is done with Ld
             Ld[: p1 - p0].copy_(pinned[: p1 - p0], non_blocking=True)
+            torch.cuda.synchronize()  # ... and the copy with the pinned buffer before the next block is generated into it
             sie.sie_dfmp2_transform(plan, ws, C_occ, C_vir, Ld[: p1 - p0], p0, p1)
         E = torch.zeros(1, dtype=torch.float64, device="cuda")
         G = torch.zeros(spec.nocc, spec.nocc, dtype=torch.float64, device="cuda")
