@@ -104,6 +104,12 @@ RAGGED = [
     (72, 75, 0, 90),
     (120, 140, 0, 200),
     (128, 130, 4, 72),
+    # many virtual blocks per tile (ta = 64, 42, 18, 4 with a ragged last block), one block of 127 rows
+    (2, 70, 0, 24),
+    (3, 200, 1, 9),
+    (7, 300, 0, 40),
+    (30, 41, 0, 88),
+    (127, 3, 0, 16),
 ]
 
 
