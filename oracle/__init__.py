@@ -30,6 +30,8 @@ def lib() -> ctypes.CDLL:
         L.sie_oracle_transform.restype = ctypes.c_int
         L.sie_oracle_pair_G.argtypes = [ctypes.c_int] * 3 + [dp, dp, dp, ctypes.c_int, ctypes.c_int, dp]
         L.sie_oracle_pair_G.restype = ctypes.c_int
+        L.sie_oracle_rdm_occ.argtypes = [ctypes.c_int] * 3 + [dp, dp, dp, dp]
+        L.sie_oracle_rdm_occ.restype = ctypes.c_int
         L.sie_oracle_trace.argtypes = [ctypes.c_int, dp, dp]
         L.sie_oracle_trace.restype = ctypes.c_double
         _lib = L
@@ -98,6 +100,18 @@ def pair_G(B, e_occ, e_vir, j0: int = 0, j1: Optional[int] = None) -> np.ndarray
     if rc != 0:
         raise MemoryError("sie_oracle_pair_G")
     return G
+
+
+def rdm_occ(B, e_occ, e_vir) -> np.ndarray:
+    """Occupied block of the MP2 1-RDM, gamma_ij of PAPER.md Eq. S18 (L357): [nocc][nocc]."""
+    B, e_occ, e_vir = _c(B), _c(e_occ), _c(e_vir)
+    nocc, nvir, naux = B.shape
+    assert e_occ.shape == (nocc,) and e_vir.shape == (nvir,)
+    g = np.empty((nocc, nocc))
+    rc = lib().sie_oracle_rdm_occ(nocc, nvir, naux, _p(B), _p(e_occ), _p(e_vir), _p(g))
+    if rc != 0:
+        raise MemoryError("sie_oracle_rdm_occ")
+    return g
 
 
 def trace(P_frag, G) -> float:

@@ -25,6 +25,9 @@
  * of O4 uses 8 explicit partial sums (still a plain loop); the (a,b), j and trace accumulations are
  * carried in long double so the oracle's own rounding sits far below the GPU's.
  *
+ * NEXT-1 addition at the end of this file: O8 gamma_ij, occupied block of the MP2 1-RDM (Eq. S18), pinned in
+ * tests/test_oracle_rdm_pins.py.
+ *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): hand-worked 2x1 and 1x1 cases
  * (tests/golden/handworked.txt), closed form o=v=1, P=I == textbook closed-shell MP2 from brute-force
  * four-index integrals, fragment additivity, invariances, scalings.  No function here is unpinned.
@@ -186,4 +189,49 @@ double sie_oracle_trace(int nocc, const double* P, const double* G) {
             e += (long double)p * (long double)G[(size_t)ip * nocc + i];
         }
     return (double)e;
+}
+
+/*
+ * NEXT-1: occupied block of the MP2 one-particle reduced density matrix, PAPER.md Eq. S18 (L357):
+ *     gamma_ij = 2 delta_ij - 2 sum_k sum_ab t_ik^ab ( 2 t_jk^ab - t_jk^ba ),   t_ik^ab = (ia|kb) / (e_i + e_k - e_a - e_b)
+ * (Eq. S15-S16, with the sign folded into the denominator as in O5; gamma is quadratic in t).
+ *   B [nocc][nvir][naux], e_occ[nocc], e_vir[nvir]; gamma [nocc][nocc] row-major, OVERWRITTEN.
+ * Loops in the paper's order: for each k, the amplitudes t_ik^ab of all i, then every (i, j) pair.  Returns 0, or 1 on
+ * allocation failure.  Pins: tests/test_oracle_pins.py (closed form o=v=1, brute force from explicit four-index
+ * amplitudes, gamma_ii = 2 + dE/de_i against the pinned energy, symmetry, positive semi-definiteness of 2 - gamma).
+ */
+int sie_oracle_rdm_occ(int nocc, int nvir, int naux, const double* B, const double* e_occ, const double* e_vir,
+                       double* gamma) {
+    const size_t vv = (size_t)nvir * nvir;
+    double* Tk = (double*)malloc(sizeof(double) * (size_t)nocc * vv);      /* t_ik^ab for all i at fixed k */
+    long double* Gl = (long double*)calloc((size_t)nocc * nocc, sizeof(long double));
+    if (!Tk || !Gl) { free(Tk); free(Gl); return 1; }
+    for (int k = 0; k < nocc; ++k) {
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int i = 0; i < nocc; ++i)
+            for (int a = 0; a < nvir; ++a) {
+                const double* bia = B + ((size_t)i * nvir + a) * naux;
+                double* t = Tk + (size_t)i * vv + (size_t)a * nvir;
+                for (int b = 0; b < nvir; ++b)
+                    t[b] = dot8(bia, B + ((size_t)k * nvir + b) * naux, naux) / (e_occ[i] + e_occ[k] - e_vir[a] - e_vir[b]);
+            }
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int i = 0; i < nocc; ++i)
+            for (int j = 0; j < nocc; ++j) {
+                const double* Ti = Tk + (size_t)i * vv;
+                const double* Tj = Tk + (size_t)j * vv;
+                long double s = 0.0L;
+                for (int a = 0; a < nvir; ++a)
+                    for (int b = 0; b < nvir; ++b)
+                        s += (long double)Ti[(size_t)a * nvir + b] *
+                             (2.0L * (long double)Tj[(size_t)a * nvir + b] - (long double)Tj[(size_t)b * nvir + a]);
+                Gl[(size_t)i * nocc + j] += s;
+            }
+    }
+    for (int i = 0; i < nocc; ++i)
+        for (int j = 0; j < nocc; ++j)
+            gamma[(size_t)i * nocc + j] = (double)((i == j ? 2.0L : 0.0L) - 2.0L * Gl[(size_t)i * nocc + j]);
+    free(Tk);
+    free(Gl);
+    return 0;
 }
