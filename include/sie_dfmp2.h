@@ -88,6 +88,20 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
                      const double* P_frag, double* E_out, double* G_out, void* cuda_stream);
 
 /*
+ * 3b. sie_dfmp2_rdm_occ — NEXT-1: occupied block of the MP2 one-particle reduced density matrix of the
+ *    cluster, PAPER.md Eq. S18 (L357) with the amplitudes of Eq. S15-S16 (L348-L351):
+ *        gamma_ij = 2 delta_ij - 2 sum_k sum_ab t_ik^ab (2 t_jk^ab - t_jk^ba),   t_ik^ab = (ia|kb) / (e_i + e_k - e_a - e_b)
+ *    (the matrix whose eigenvectors rank the occupied bath natural orbitals).  Same fused kernel as the energy: the
+ *    (ia|kb) tile is turned into amplitudes in shared memory and contracted with itself; nothing reaches HBM.
+ *      e_occ [nocc], e_vir [nvir]; gamma_out [nocc][nocc] row-major (symmetric), REQUIRED;
+ *      trace_out: 1 double or NULL, receives Tr gamma (the electron count left in the occupied block).
+ *    Pointers device or host per SIE_FLAG_HOST_IO, call order and errors as sie_dfmp2_energy; may be called before or
+ *    after sie_dfmp2_energy on the same transformed workspace, any number of times.
+ */
+int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir,
+                      double* gamma_out, double* trace_out, void* cuda_stream);
+
+/*
  * 4. sie_dfmp2_batch — many independent clusters (no contraction across clusters) in one
  *    scheduled submission: per-cluster transforms, then ONE persistent pair kernel whose CTAs walk a
  *    static, cost-balanced list of (cluster, tile) work items, then one reduction launch (step A7).

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     sie_dfmp2_batch_query,
     sie_dfmp2_destroy,
     sie_dfmp2_energy,
+    sie_dfmp2_rdm_occ,
     sie_dfmp2_plan,
     sie_dfmp2_plan_info,
     sie_dfmp2_plan_timing,

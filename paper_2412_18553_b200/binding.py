@@ -22,6 +22,7 @@ EXPORTS = (
     "sie_dfmp2_plan",
     "sie_dfmp2_transform",
     "sie_dfmp2_energy",
+    "sie_dfmp2_rdm_occ",
     "sie_dfmp2_batch",
     "sie_dfmp2_destroy",
     "sie_dfmp2_strerror",
@@ -80,6 +81,8 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_transform.restype = ci
         L.sie_dfmp2_energy.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
         L.sie_dfmp2_energy.restype = ci
+        L.sie_dfmp2_rdm_occ.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.sie_dfmp2_rdm_occ.restype = ci
         L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
         L.sie_dfmp2_batch.restype = ci
         L.sie_dfmp2_destroy.argtypes = [vp]
@@ -144,6 +147,16 @@ def sie_dfmp2_transform(plan: int, workspace: torch.Tensor, C_occ, C_vir, L_pack
             plan, workspace.data_ptr(), _ptr(C_occ, host, "C_occ"), _ptr(C_vir, host, "C_vir"),
             _ptr(L_packed_block, host, "L_packed_block"), p0, p1, _stream_ptr(stream)),
         "sie_dfmp2_transform",
+    )
+
+
+def sie_dfmp2_rdm_occ(plan: int, workspace: torch.Tensor, e_occ, e_vir, gamma_out, trace_out=None, *, host=False, stream=None) -> None:
+    """Occupied block of the MP2 1-RDM (PAPER.md Eq. S18) on the transformed workspace; marshalling only."""
+    _check(
+        _lib().sie_dfmp2_rdm_occ(
+            plan, workspace.data_ptr(), _ptr(e_occ, host, "e_occ"), _ptr(e_vir, host, "e_vir"), _ptr(gamma_out, host, "gamma_out"),
+            _ptr(trace_out, host, "trace_out"), _stream_ptr(stream)),
+        "sie_dfmp2_rdm_occ",
     )
 
 
@@ -264,6 +277,16 @@ class ClusterSolver:
             E, G = E.pin_memory(), (G.pin_memory() if G is not None else None)
         sie_dfmp2_energy(self.plan, self.workspace, e_occ, e_vir, P_frag, E, G, host=self.host, stream=stream)
         return E, G
+
+    def rdm_occ(self, e_occ, e_vir, stream=None):
+        """-> (gamma [nocc][nocc], Tr gamma)"""
+        dev = "cpu" if self.host else self.device
+        g = torch.empty(self.nocc, self.nocc, dtype=torch.float64, device=dev)
+        tr = torch.empty(1, dtype=torch.float64, device=dev)
+        if self.host:
+            g, tr = g.pin_memory(), tr.pin_memory()
+        sie_dfmp2_rdm_occ(self.plan, self.workspace, e_occ, e_vir, g, tr, host=self.host, stream=stream)
+        return g, tr
 
     def timing(self) -> dict:
         return sie_dfmp2_plan_timing(self.plan)

@@ -552,9 +552,9 @@ int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_
     return SIE_OK;
 }
 
-int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, const double* P_frag,
-                     double* E_out, double* G_out, void* cuda_stream) {
-    if (!plan || !workspace || !e_occ || !e_vir || !E_out) return SIE_EINVAL;
+static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, const double* P_frag,
+                       double* E_out, double* G_out, void* cuda_stream, int mode) {
+    if (!plan || !workspace || !e_occ || !e_vir || (!E_out && mode == 0)) return SIE_EINVAL;
     sie_dfmp2_plan_s& p = *plan;
     if (p.covered_rows != p.naux || p.c_ready_ws != workspace) return SIE_ESTATE;
     SIE_TRY(check_device());
@@ -565,6 +565,7 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
 
     const double *de_occ = e_occ, *de_vir = e_vir, *dP = P_frag;
     double *dE = E_out, *dG = G_out;
+    if (!dE) dE = reinterpret_cast<double*>(ws + p.off_rc + 128);  // mode 1 without a trace output: spare bytes behind the descriptor
     double* io = reinterpret_cast<double*>(ws + p.off_io);
     if (host) {
         if (p.flags & SIE_FLAG_VALIDATE) SIE_TRY(check_gap_host(e_occ, e_vir, o, v));
@@ -592,11 +593,12 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
     rc.E_out = dE;
     rc.G_out = dG;
     rc.o = o;
+    rc.mode = mode;
     if (p.ref) {
         double* G = reinterpret_cast<double*>(ws + p.off_refG);
         {
             ProfSpan ps(p.prof, ST_REF, st);
-            SIE_TRY(ref_pair(Bmat, o, v, p.naux, p.naux_ld, de_occ, de_vir, reinterpret_cast<double*>(ws + p.off_refVj), G, st));
+            SIE_TRY(ref_pair(Bmat, o, v, p.naux, p.naux_ld, de_occ, de_vir, reinterpret_cast<double*>(ws + p.off_refVj), G, mode, st));
         }
         rc.gpart = G;
         rc.o8 = o;
@@ -606,6 +608,7 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
         PairCluster pc;
         SIE_TRY(fill_pair_cluster(p, Bmat, de_occ, de_vir, gpart, p.kp, pc));
         pc.gate = 1;  // one cluster: all tiles cost the same, keep the CTAs in K-lockstep for L2
+        pc.mode = mode;
         SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
         SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
         SIE_CUDA(cudaMemsetAsync(ws + p.off_tiles + p.tiles.size() * sizeof(PairTile), 0, 256, st));
@@ -625,11 +628,22 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
         SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
     }
     if (host) {
-        SIE_CUDA(cudaMemcpyAsync(E_out, dE, 8, cudaMemcpyDeviceToHost, st));
+        if (E_out) SIE_CUDA(cudaMemcpyAsync(E_out, dE, 8, cudaMemcpyDeviceToHost, st));
         if (G_out) SIE_CUDA(cudaMemcpyAsync(G_out, dG, (size_t)o * o * 8, cudaMemcpyDeviceToHost, st));
         SIE_CUDA(cudaStreamSynchronize(st));
     }
     return SIE_OK;
+}
+
+int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, const double* P_frag,
+                     double* E_out, double* G_out, void* cuda_stream) {
+    return energy_impl(plan, workspace, e_occ, e_vir, P_frag, E_out, G_out, cuda_stream, 0);
+}
+
+int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, double* gamma_out,
+                      double* trace_out, void* cuda_stream) {
+    if (!gamma_out) return SIE_EINVAL;
+    return energy_impl(plan, workspace, e_occ, e_vir, nullptr, trace_out, gamma_out, cuda_stream, 1);
 }
 
 int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes, size_t* needed,
@@ -819,7 +833,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             {
                 ProfSpan ps(prof, ST_REF, st);
                 SIE_TRY(ref_pair(reinterpret_cast<const double*>(wk + p.off_B), p.o, p.v, p.naux, p.naux_ld, de_occ[k], de_vir[k],
-                                 reinterpret_cast<double*>(ws + off_refVj), G, st));
+                                 reinterpret_cast<double*>(ws + off_refVj), G, 0, st));
             }
             rcs[k].gpart = G;
             rcs[k].o8 = p.o;

@@ -72,7 +72,7 @@ __global__ void ref_vj_kernel(const double* __restrict__ B, int o, int v, int na
 // G[i'][i] += sum_ab Vj[i'][a][b] / (e_i' + e_j - e_a - e_b) * (2 Vj[i][a][b] - Vj[i][b][a]); one CTA per (i', i).
 __global__ void __launch_bounds__(256) ref_g_kernel(const double* __restrict__ Vj, int o, int v, int j,
                                                     const double* __restrict__ e_occ, const double* __restrict__ e_vir,
-                                                    double* __restrict__ G) {
+                                                    double* __restrict__ G, int mode) {
     const int ip = blockIdx.y, i = blockIdx.x;
     const double* Vp = Vj + (size_t)ip * v * v;
     const double* Vi = Vj + (size_t)i * v * v;
@@ -81,7 +81,9 @@ __global__ void __launch_bounds__(256) ref_g_kernel(const double* __restrict__ V
     for (int ab = threadIdx.x; ab < v * v; ab += 256) {
         const int a = ab / v, b = ab - a * v;
         const double D = (eij - e_vir[a]) - e_vir[b];
-        s = fma(Vp[ab] / D, 2.0 * Vi[ab] - Vi[(size_t)b * v + a], s);
+        const double w = 2.0 * Vi[ab] - Vi[(size_t)b * v + a];
+        // mode 1 (Eq. S18): the second factor is an amplitude too, t_{ij}^{ab} and t_{ij}^{ba} share D_{ij}^{ab}
+        s = fma(Vp[ab] / D, mode ? w / (((e_occ[i] + e_occ[j]) - e_vir[a]) - e_vir[b]) : w, s);
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
@@ -98,13 +100,13 @@ __global__ void __launch_bounds__(256) ref_g_kernel(const double* __restrict__ V
 size_t ref_vj_bytes(int o, int v) { return (size_t)o * v * v * sizeof(double); }
 
 int ref_pair(const double* B, int o, int v, int naux, int naux_ld, const double* e_occ, const double* e_vir, double* Vj,
-             double* G, cudaStream_t st) {
+             double* G, int mode, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(G, 0, (size_t)o * o * sizeof(double), st);
     if (e != cudaSuccess) return set_cuda_error(e);
     for (int j = 0; j < o; ++j) {
         ref_vj_kernel<<<dim3((v + 15) / 16, (v + 15) / 16, o), dim3(16, 16), 0, st>>>(B, o, v, naux, naux_ld, j, Vj);
         note_launch();
-        ref_g_kernel<<<dim3(o, o), 256, 0, st>>>(Vj, o, v, j, e_occ, e_vir, G);
+        ref_g_kernel<<<dim3(o, o), 256, 0, st>>>(Vj, o, v, j, e_occ, e_vir, G, mode);
         note_launch();
     }
     e = cudaGetLastError();

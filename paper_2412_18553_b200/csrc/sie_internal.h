@@ -43,6 +43,7 @@ struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (g
     uint32_t tx_bytes;             // bytes of both operand boxes of one stage
     int t8;                        // tile edge in rows of B: ceil8(ta * o) <= 128
     int gate;                      // 1: producers keep the CTAs of a round in K-lockstep (equal-cost tiles only)
+    int mode;                      // 0: G of the energy path; 1: Gamma of the occupied 1-RDM block (amplitudes on both sides)
 };
 struct PairTile {                  // 8 bytes
     int cluster;
@@ -60,7 +61,8 @@ struct ReduceCluster {             // per cluster, device array
     const double* P;               // [o][o] or nullptr
     double* E_out;                 // 1
     double* G_out;                 // [o][o] or nullptr
-    int o, o8, nslots, pad_;
+    int o, o8, nslots;
+    int mode;                      // 0: G_out = G, E_out = sum P o G^T; 1: G_out = 2 delta - 2 Gamma, E_out = its trace
 };
 int launch_reduce(const ReduceCluster* d_rc, int ncluster, cudaStream_t st);
 
@@ -69,7 +71,7 @@ int launch_reduce(const ReduceCluster* d_rc, int ncluster, cudaStream_t st);
 int ref_transform(const double* C_occ, const double* C_vir, const double* Lp_block, int nao, int o, int v, int p0, int p1,
                   double* H /*[(p1-p0)][o][nao]*/, double* B, int naux_ld, cudaStream_t st);
 int ref_pair(const double* B, int o, int v, int naux, int naux_ld, const double* e_occ, const double* e_vir,
-             double* Vj /*[o][v][v]*/, double* G /*[o][o]*/, cudaStream_t st);
+             double* Vj /*[o][v][v]*/, double* G /*[o][o]*/, int mode /*0 G, 1 Gamma*/, cudaStream_t st);
 size_t ref_vj_bytes(int o, int v);
 
 // ---- probes.cu ---------------------------------------------------------------------------------
