@@ -384,6 +384,33 @@ def run_gpu(args) -> None:
             best = max(best, tf)
         probes[name] = best
 
+    # ---- NEXT-1 (optional): occupied MP2 1-RDM block on the same transformed B, same fused kernel in amplitude mode
+    next1 = None
+    if args.rdm and single:
+        s0, d0 = specs[0], devc[0]
+        plan, nb = sie.sie_dfmp2_plan(s0.nao, s0.nocc, s0.nvir, s0.naux, 0, 0)
+        ws1 = sie.alloc_workspace(nb, dev)
+        sie.sie_dfmp2_transform(plan, ws1, d0["C_occ"], d0["C_vir"], d0["L_packed"], 0, s0.naux)
+        gam = torch.zeros(s0.nocc, s0.nocc, dtype=torch.float64, device=dev)
+        tr = torch.zeros(1, dtype=torch.float64, device=dev)
+        for _ in range(max(1, min(args.warmup, 2))):
+            sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = max(1, min(args.steps, 3))
+        ev0.record()
+        for _ in range(reps):
+            sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms_rdm = ev0.elapsed_time(ev1) / reps
+        f_rdm = alg_flops(s0)["pair_kernel"]  # same contraction count: SYRK of B plus two o^3 products per virtual pair
+        next1 = {"call": "sie_dfmp2_rdm_occ", "ms": ms_rdm, "tflops": f_rdm / (ms_rdm * 1e-3) * 1e-12,
+                 "trace_gamma": float(tr.cpu()[0]), "algorithmic_flops": f_rdm, "includes": "pair kernel (amplitude mode) + reduce"}
+        sie.sie_dfmp2_destroy(plan)
+        del ws1, gam
+        torch.cuda.empty_cache()
+
     # ---- arm 2: end to end through the C ABI with host buffers (H2D of every input + D2H of E, G inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -462,6 +489,9 @@ def run_gpu(args) -> None:
             "roofline": roofline, "transform": transform, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": launches,
             "workspace_bytes": ws_bytes, "input_gen_s": t_gen,
         }
+        if next1 is not None:
+            next1["frac_of_fp64_peak"] = next1["tflops"] / peak_probe if peak_probe else None
+            line["next1_rdm_occ"] = next1
         if e2e is None and not args.no_e2e:
             e2e = {"value": f_job / (ms_e2e * 1e-3) * 1e-12, "unit": UNIT, "ms_per_step": ms_e2e,
                    "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes, "steps": e_steps,
@@ -542,6 +572,7 @@ def main() -> None:
     ap.add_argument("--impl", default="sie", choices=["sie", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end arm")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle leg")
+    ap.add_argument("--rdm", action="store_true", help="also time sie_dfmp2_rdm_occ (NEXT-1: occupied MP2 1-RDM block) on the same B")
     ap.add_argument("--streamed", action="store_true", help="feed the packed integrals in aux blocks generated on the fly "
                                                              "(sweep points that do not fit in HBM; not a bench line)")
     ap.add_argument("--stream-gb", type=float, default=8.0, help="size of one streamed aux block in GB")

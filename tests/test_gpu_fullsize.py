@@ -47,8 +47,9 @@ def _sparse_case(spec, rows, virt):
     info = s.info()
     s.transform(cu(x.C_occ), cu(C_vir), L, 0, spec.naux)  # one call over [0, naux), as bench.py does
     E, G = s.energy(cu(x.e_occ), cu(x.e_vir), cu(x.P_frag))
+    gam, _ = s.rdm_occ(cu(x.e_occ), cu(x.e_vir))  # NEXT-1 on the same B, same special case (0 / D == 0 exactly)
     torch.cuda.synchronize()
-    E, G = float(E.cpu()[0]), G.cpu().numpy()
+    E, G, gam = float(E.cpu()[0]), G.cpu().numpy(), gam.cpu().numpy()
     s.close()
     del L
     torch.cuda.empty_cache()
@@ -56,6 +57,9 @@ def _sparse_case(spec, rows, virt):
     Bor = oracle.transform(x.C_occ, np.ascontiguousarray(x.C_vir[:, virt]), Lsub)
     Gor = oracle.pair_G(Bor, x.e_occ, np.ascontiguousarray(x.e_vir[virt]))
     Eor = oracle.trace(x.P_frag, Gor)
+    gam_or = oracle.rdm_occ(Bor, x.e_occ, np.ascontiguousarray(x.e_vir[virt]))
+    assert np.max(np.abs(gam - gam_or)) <= G_ATOL * max(1.0, float(np.max(np.abs(gam_or))))
+    assert np.max(np.abs(gam_or - 2.0 * np.eye(spec.nocc))) > 1e-6  # the special case is not trivially the identity
     return info, E, G, Eor, Gor
 
 
