@@ -616,7 +616,7 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
         {
             ProfSpan ps(p.prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc),
-                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8, st));
+                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8, mode, st));
         }
         rc.gpart = gpart;
         rc.o8 = p.o8;
@@ -822,7 +822,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_CUDA(cudaMemsetAsync(ws + off_tiles + tiles.size() * sizeof(PairTile), 0, 256, st));
             ProfSpan ps(prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
-                                (int)tiles.size(), ncta, tmax, st));
+                                (int)tiles.size(), ncta, tmax, 0, st));
         }
         // reference-path clusters (nocc > 128 or SIE_FLAG_REFERENCE): per-j kernels, one cluster at a time
         for (int k = 0; k < ncluster; ++k) {

@@ -54,7 +54,8 @@ struct PairGeom {                  // tile configuration facts for host-side pla
 };
 PairGeom pair_geom();
 size_t pair_smem_bytes();
-int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, cudaStream_t st);
+// mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma); one mode per launch
+int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, int mode, cudaStream_t st);
 
 struct ReduceCluster {             // per cluster, device array
     const double* gpart;           // [nslots][o8*o8]
