@@ -437,7 +437,10 @@ int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const doubl
     return SIE_OK;
 }
 
-constexpr int BATCH_LANES = 4;
+#ifndef SIE_BATCH_LANES
+#define SIE_BATCH_LANES 4
+#endif
+constexpr int BATCH_LANES = SIE_BATCH_LANES;
 
 // side streams of one batch call: forked from / joined into the caller's stream with events
 struct LaneStreams {
