@@ -344,7 +344,6 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
         return SIE_OK;
     }
     const int tm1 = gemm_tm_for(o), tm2 = gemm_tm_for(v);
-    const int nvb = (nao + 127) / 128;
     const int kblocks = (nao + 7) / 8;
     CUtensorMap mapCo, mapCv;
     SIE_TRY(make_tensor_map_3d(&mapCo, sc.CoT, nao, o, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * o, 8, tm1, 1));
@@ -374,20 +373,23 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
             ProfSpan ps(prof, ST_UNPACK, st);
             SIE_TRY(launch_unpack(Lq, pb, nao, sc.Lfull, p.nao_ld, st));
         }
-        // A1: H[i][P][nu] = sum_mu CoT[i][mu] * Lfull[P][nu][mu]
+        // A1: H[i][P][nu] = sum_mu CoT[i][mu] * Lfull[P][nu][mu].  The pb * nao rows (P, nu) of the unpacked block are
+        // contiguous, so the N dimension is tiled over the flat row index: no per-P padding of nao to 128
         CUtensorMap mapL, mapH;
-        SIE_TRY(make_tensor_map_3d(&mapL, sc.Lfull, nao, nao, pb, (uint64_t)p.nao_ld * 8, (uint64_t)nao * p.nao_ld * 8, 8, 128, 1));
+        const uint64_t lrows = (uint64_t)pb * nao;
+        SIE_TRY(make_tensor_map_3d(&mapL, sc.Lfull, nao, lrows, 1, (uint64_t)p.nao_ld * 8, lrows * p.nao_ld * 8, 8, 128, 1));
         GemmOut o1;
         o1.base = sc.H;
         o1.ld_m = (long long)pb * p.nao_ld;
         o1.M = o;
-        o1.inner = nvb * 128;
+        o1.inner = nao;
         o1.valid_inner = nao;
         o1.stride_outer = p.nao_ld;
-        o1.n_lin_total = (long long)pb * nvb * 128;
+        o1.n_lin_total = (long long)lrows;
+        const int n1_tiles = (int)((lrows + 127) / 128);
         {
             ProfSpan ps(prof, ST_T1, st);
-            SIE_TRY(launch_gemm_tn(tm1, mapCo, mapL, 1, pb * nvb, nvb, (long long)nvb * 128, kblocks, o1, p.num_sms, st));
+            SIE_TRY(launch_gemm_tn(tm1, mapCo, mapL, 1, n1_tiles, n1_tiles, 0, kblocks, o1, p.num_sms, st));
         }
         // A2: B[a][i][q0+P] = sum_nu CvT[a][nu] * H[(i,P)][nu]
         SIE_TRY(make_tensor_map_3d(&mapH, sc.H, nao, (uint64_t)o * pb, 1, (uint64_t)p.nao_ld * 8,
