@@ -55,7 +55,9 @@ enum {
     SIE_FLAG_VALIDATE = 1u,  /* energy/batch copy e_occ,e_vir to the host (synchronising) and check the gap */
     SIE_FLAG_REFERENCE = 2u, /* use the simple FP64-FMA reference kernels (any nocc; slow; cross-check path) */
     SIE_FLAG_HOST_IO = 4u,   /* data pointers are HOST pointers; the library stages H2D/D2H copies */
-    SIE_FLAG_PROFILE = 8u    /* bracket every launch group with CUDA events; read with *_timing (below) */
+    SIE_FLAG_PROFILE = 8u,   /* bracket every launch group with CUDA events; read with *_timing (below) */
+    SIE_FLAG_RDM_OCC = 16u   /* sie_dfmp2_batch only: compute the occupied 1-RDM block of every cluster instead of the
+                                energy (3b): G_out receives gamma, E_out receives Tr gamma, P_frag is ignored */
 };
 
 /*

@@ -6,6 +6,7 @@ this package is its thin Python binding.  Nothing here computes on the CPU and n
 from .binding import (  # noqa: F401
     SIE_FLAG_HOST_IO,
     SIE_FLAG_PROFILE,
+    SIE_FLAG_RDM_OCC,
     SIE_FLAG_REFERENCE,
     SIE_FLAG_VALIDATE,
     ClusterSolver,

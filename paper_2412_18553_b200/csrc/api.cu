@@ -654,8 +654,9 @@ int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_oc
 int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes, size_t* needed,
                     unsigned flags, void* cuda_stream) {
     if (ncluster < 0 || (ncluster > 0 && !clusters)) return SIE_EINVAL;
-    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE)) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_OCC)) return SIE_EINVAL;
     const bool host = flags & SIE_FLAG_HOST_IO;
+    const int mode = (flags & SIE_FLAG_RDM_OCC) ? 1 : 0;
     const bool query = (workspace == nullptr || workspace_bytes == 0);
     if (query && !needed) return SIE_EINVAL;
     if (ncluster == 0) {  // nothing to schedule: no workspace, no launch
@@ -672,7 +673,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             const sie_dfmp2_cluster_t& cl = clusters[k];
             if (!query && (!cl.C_occ || !cl.C_vir || !cl.L_packed || !cl.e_occ || !cl.e_vir || !cl.E_out)) return SIE_EINVAL;
             sie_dfmp2_plan_s& p = plans[k];
-            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~(SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE), false));
+            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~(SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_OCC), false));
             off_cl[k] = c.take(p.total);
             if (!p.ref) {
                 max_CoT = std::max(max_CoT, (size_t)p.o * p.nao_ld * 8);
@@ -795,6 +796,8 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             rcs[k].E_out = dE[k];
             rcs[k].G_out = dG[k];
             rcs[k].o = p.o;
+            rcs[k].mode = mode;
+            if (mode) rcs[k].P = nullptr;
         }
         if (nlanes > 1) SIE_TRY(ls.join(st));
         // ---- stage 2: one persistent pair launch over all (cluster, tile) items, most expensive tiles first
@@ -827,7 +830,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_CUDA(cudaMemsetAsync(ws + off_tiles + tiles.size() * sizeof(PairTile), 0, 256, st));
             ProfSpan ps(prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
-                                (int)tiles.size(), ncta, tmax, 0, st));
+                                (int)tiles.size(), ncta, tmax, mode, st));
         }
         // reference-path clusters (nocc > 128 or SIE_FLAG_REFERENCE): per-j kernels, one cluster at a time
         for (int k = 0; k < ncluster; ++k) {
@@ -838,7 +841,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             {
                 ProfSpan ps(prof, ST_REF, st);
                 SIE_TRY(ref_pair(reinterpret_cast<const double*>(wk + p.off_B), p.o, p.v, p.naux, p.naux_ld, de_occ[k], de_vir[k],
-                                 reinterpret_cast<double*>(ws + off_refVj), G, 0, st));
+                                 reinterpret_cast<double*>(ws + off_refVj), G, mode, st));
             }
             rcs[k].gpart = G;
             rcs[k].o8 = p.o;

@@ -76,3 +76,27 @@ def test_closed_form_o1_v1_on_gpu():
     B = oracle.transform(x.C_occ, x.C_vir, x.L_packed())
     t = float(np.sum(B * B)) / (2 * x.e_occ[0] - 2 * x.e_vir[0])
     assert g[0, 0] == pytest.approx(2.0 - 2.0 * t * t, rel=1e-13) and tr == pytest.approx(g[0, 0], rel=1e-15)
+
+
+@pytest.mark.parametrize("flags", [0, binding.SIE_FLAG_HOST_IO, binding.SIE_FLAG_REFERENCE], ids=["device", "host_io", "reference"])
+def test_batch_with_rdm_flag(flags):
+    """sie_dfmp2_batch(..., SIE_FLAG_RDM_OCC): gamma of every cluster in G_out, Tr gamma in E_out."""
+    specs = [ClusterSpec(58, k, o + v, o, v, naux, 1, "std") for k, (o, v, naux) in enumerate([(16, 128, 100), (7, 30, 41), (33, 64, 72), (24, 50, 90)])]
+    host = bool(flags & binding.SIE_FLAG_HOST_IO)
+    to = (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()) if host else (lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda())
+    mk = (lambda *sh: torch.zeros(*sh, dtype=torch.float64).pin_memory()) if host else (lambda *sh: torch.zeros(*sh, dtype=torch.float64, device="cuda"))
+    xs, cl = [], []
+    for sp in specs:
+        x = make_cluster(sp)
+        xs.append(x)
+        cl.append(dict(nao=sp.nao, nocc=sp.nocc, nvir=sp.nvir, naux=sp.naux, C_occ=to(x.C_occ), C_vir=to(x.C_vir), L_packed=to(x.L_packed()),
+                       e_occ=to(x.e_occ), e_vir=to(x.e_vir), P_frag=to(x.P_frag), E_out=mk(1), G_out=mk(sp.nocc, sp.nocc)))
+    fl = flags | binding.SIE_FLAG_RDM_OCC
+    ws = sie.alloc_workspace(sie.sie_dfmp2_batch_query(cl, fl))
+    sie.sie_dfmp2_batch(cl, ws, fl)
+    torch.cuda.synchronize()
+    for x, c in zip(xs, cl):
+        gor = oracle.rdm_occ(oracle.transform(x.C_occ, x.C_vir, x.L_packed()), x.e_occ, x.e_vir)
+        g = c["G_out"].cpu().numpy()
+        assert np.max(np.abs(g - gor)) <= ATOL * max(1.0, float(np.max(np.abs(gor))))
+        assert abs(float(c["E_out"].cpu()[0]) - np.trace(gor)) <= 1e-10 * max(1.0, abs(np.trace(gor)))
