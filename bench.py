@@ -36,11 +36,25 @@ from workloads import ClusterSpec, config_specs, make_cluster  # noqa: E402
 
 METRIC = "DF-MP2 cluster energy: FP64 TFLOP/s (algorithmic) & % of FP64 peak; clusters/s (batched)"
 UNIT = "TFLOP/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE pair_kernel launch, from the committed ncu --set full
-# captures under profiles/ (file named beside each number); None = not captured for that workload.
-NCU_PAIR_TRAFFIC_BYTES = {
-    "config3": 529.222e9 + 85.369e9,              # profiles/r01_ncu_pair_rev3_config3.md
-}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE pair_kernel launch are read from this table of the committed
+# ncu --set full captures (one row per workload: workload,dram_read_bytes,dram_write_bytes,capture file).
+NCU_TRAFFIC_TABLE = os.path.join(ROOT, "profiles", "pair_kernel_dram_traffic.csv")
+
+
+def ncu_pair_traffic(workload: str):
+    """-> (bytes per launch or None, name of the profiles/ capture it comes from or None)."""
+    try:
+        with open(NCU_TRAFFIC_TABLE) as fh:
+            rows = [ln.strip().split(",") for ln in fh if ln.strip() and not ln.startswith("#")]
+    except OSError:
+        return None, None
+    hit = None
+    for r in rows:
+        if len(r) >= 4 and r[0] == workload:
+            hit = r  # the last row of a workload is the newest capture
+    if hit is None:
+        return None, None
+    return float(hit[1]) + float(hit[2]), hit[3]
 
 
 # ------------------------------------------------------------------------------------------------ flop model
@@ -171,7 +185,7 @@ def oracle_sample(spec: ClusterSpec, n_aux_rows: int = 96, n_j: int = 16, v_sub:
     return total, t_tr + t_pair, desc
 
 
-def oracle_workload_seconds(specs, budget_per_cluster=None):
+def oracle_workload_seconds(specs):
     """Extrapolated oracle seconds for a list of clusters (a batch is sampled on its largest cluster)."""
     import oracle
 
@@ -245,50 +259,73 @@ def reduce_over_ranks(ms: float, units: float, world: int, device) -> tuple:
 
 
 # ------------------------------------------------------------------------------------------------ GPU arm
-def run_gpu(args) -> None:
-    import torch
-    import torch.distributed as dist
+class GpuBench:
+    """Everything run_gpu needs to time workloads in ONE process: device, ranks, event timing, clock sampling."""
 
-    import paper_2412_18553_b200 as sie  # raises if libsie_dfmp2.so is missing: there is no fallback
+    def __init__(self):
+        import torch
+        import torch.distributed as dist
 
-    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU path. Use --impl reference for the CPU oracle.")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        import paper_2412_18553_b200 as sie  # raises if libsie_dfmp2.so is missing: there is no fallback
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
+        self.torch, self.dist, self.sie = torch, dist, sie
+        self.rank, self.world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+        local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU path. Use --impl reference for the CPU oracle.")
+        torch.cuda.set_device(local)
+        self.dev = torch.device("cuda", local)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=self.dev)
+        self.phys_index = local
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            try:
+                self.phys_index = int(vis.split(",")[local])
+            except (ValueError, IndexError):
+                pass
+        self.ncpu = max(1, min(32, (os.cpu_count() or 8) // max(1, self.world)))
+        self.peak = None
+        self.probes = {}
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def probe_peak(self):
+        """Live FP64 roofline denominators: register-resident DMMA / DFMA issue loops, smem-fed DMMA (best of 3)."""
+        for kind, name in ((0, "dmma_reg"), (1, "dfma_reg"), (2, "dmma_smem")):
+            best = 0.0
+            for _ in range(3):
+                tf, _ms = self.sie.sie_dfmp2_probe_fp64(kind, 40000 if kind != 2 else 10000, 2 if kind != 2 else 1)
+                best = max(best, tf)
+            self.probes[name] = best
+        self.peak = max(self.probes["dmma_reg"], self.probes["dfma_reg"])
+
+    # ---- inputs: generated once on the host (pinned when the e2e arm will read them), then uploaded
+    def make_inputs(self, specs, pinned: bool):
+        torch = self.torch
+        t0 = time.perf_counter()
+        host, devc = [], []
+        for s in specs:
+            x = make_cluster(s)
+            L = torch.empty((s.naux, s.npair), dtype=torch.float64, pin_memory=pinned)
+            x.L_block(0, s.naux, out=L.numpy(), threads=self.ncpu)
+            wrap = (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()) if pinned else (lambda a: torch.from_numpy(np.ascontiguousarray(a)))
+            h = dict(nao=s.nao, nocc=s.nocc, nvir=s.nvir, naux=s.naux, C_occ=wrap(x.C_occ), C_vir=wrap(x.C_vir), L_packed=L,
+                     e_occ=wrap(x.e_occ), e_vir=wrap(x.e_vir), P_frag=None if s.rank <= 0 else wrap(x.P_frag))
+            devc.append({k: (t.to(self.dev, non_blocking=pinned) if isinstance(t, torch.Tensor) else t) for k, t in h.items()})
+            host.append(h if pinned else None)
+            if not pinned:
+                del L, h
         torch.cuda.synchronize()
+        return host, devc, time.perf_counter() - t0
 
-    specs = workload_specs(args.workload, rank)
-    single = len(specs) == 1
-    ncpu = max(1, min(32, (os.cpu_count() or 8) // max(1, world)))
-
-    # ---- seeded inputs: generated once on the host, straight into pinned buffers (the e2e source), then uploaded
-    t_gen = time.perf_counter()
-    host, devc = [], []
-    for s in specs:
-        x = make_cluster(s)
-        L = torch.empty((s.naux, s.npair), dtype=torch.float64, pin_memory=True)
-        x.L_block(0, s.naux, out=L.numpy(), threads=ncpu)
-        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
-        h = dict(nao=s.nao, nocc=s.nocc, nvir=s.nvir, naux=s.naux, C_occ=pin(x.C_occ), C_vir=pin(x.C_vir), L_packed=L,
-                 e_occ=pin(x.e_occ), e_vir=pin(x.e_vir), P_frag=None if s.rank <= 0 else pin(x.P_frag))
-        host.append(h)
-        devc.append({k: (t.to(dev, non_blocking=True) if isinstance(t, torch.Tensor) else t) for k, t in h.items()})
-    torch.cuda.synchronize()
-    t_gen = time.perf_counter() - t_gen
-    in_bytes = sum(sum(t.numel() * 8 for t in h.values() if isinstance(t, torch.Tensor)) for h in host)
-    out_bytes = sum(8 + s.nocc * s.nocc * 8 for s in specs)
-
-    PROF = sie.SIE_FLAG_PROFILE
-
-    def make_step(data, flags):
-        """Returns (step(), results(), timing()) for the device-resident (flags=PROF) or host-I/O arm."""
+    def make_step(self, specs, data, flags):
+        """-> (step(), results(), timing(), plan info, workspace bytes) for the device-resident or the host-I/O arm.
+        One plan (host-side object) serves every step: sie_dfmp2_plan_reset between passes."""
+        sie, torch, dev = self.sie, self.torch, self.dev
         hostio = bool(flags & sie.SIE_FLAG_HOST_IO)
         mk = (lambda *sh: torch.zeros(*sh, dtype=torch.float64).pin_memory()) if hostio else (lambda *sh: torch.zeros(*sh, dtype=torch.float64, device=dev))
         outs = [(mk(1), mk(s.nocc, s.nocc)) for s in specs]
@@ -299,26 +336,23 @@ def run_gpu(args) -> None:
                 acc["ms"][k] += t["ms"][k]
                 acc["launch_groups"][k] += t["launch_groups"][k]
 
-        if single:
+        if len(specs) == 1:
             s, d = specs[0], data[0]
-            plan0, nbytes = sie.sie_dfmp2_plan(s.nao, s.nocc, s.nvir, s.naux, 0, flags)
-            info = sie.sie_dfmp2_plan_info(plan0)
-            sie.sie_dfmp2_destroy(plan0)
+            plan, nbytes = sie.sie_dfmp2_plan(s.nao, s.nocc, s.nvir, s.naux, 0, flags)
+            info = sie.sie_dfmp2_plan_info(plan)
             ws = sie.alloc_workspace(nbytes, dev)
-            pending = []
 
             def step():
-                plan, _ = sie.sie_dfmp2_plan(s.nao, s.nocc, s.nvir, s.naux, 0, flags)
+                sie.sie_dfmp2_plan_reset(plan)
                 sie.sie_dfmp2_transform(plan, ws, d["C_occ"], d["C_vir"], d["L_packed"], 0, s.naux, host=hostio)
                 sie.sie_dfmp2_energy(plan, ws, d["e_occ"], d["e_vir"], d["P_frag"], outs[0][0], outs[0][1], host=hostio)
-                pending.append(plan)
 
             def timing():
-                for plan in pending:
-                    add(sie.sie_dfmp2_plan_timing(plan))
-                    sie.sie_dfmp2_destroy(plan)
-                pending.clear()
+                add(sie.sie_dfmp2_plan_timing(plan))
                 return acc
+
+            def close():
+                sie.sie_dfmp2_destroy(plan)
         else:
             cl = [dict(d, E_out=o_[0], G_out=o_[1]) for d, o_ in zip(data, outs)]
             nbytes = sie.sie_dfmp2_batch_query(cl, flags)
@@ -334,173 +368,216 @@ def run_gpu(args) -> None:
             def timing():
                 return acc
 
+            def close():
+                pass
+
         def results():
             torch.cuda.synchronize()
             return [float(e[0]) for e, _ in outs]
 
-        return step, results, timing, info, nbytes
+        return step, results, timing, close, info, nbytes
 
-    def timed(step, timing, warmup, steps, sampler_index):
+    def timed(self, step, timing, warmup, steps):
+        sie, torch = self.sie, self.torch
         for _ in range(warmup):
             step()
-        barrier()
-        timing()  # drop the warm-up spans
-        for k in timing()["ms"]:
-            timing()["ms"][k] = 0.0
-            timing()["launch_groups"][k] = 0
+        self.barrier()
+        acc = timing()  # drop the warm-up spans
+        for k in acc["ms"]:
+            acc["ms"][k] = 0.0
+            acc["launch_groups"][k] = 0
         l0 = sie.launch_count()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        with ClockSampler(sampler_index) as cs:
+        with ClockSampler(self.phys_index) as cs:
             ev0.record()
             for _ in range(steps):
                 step()
             ev1.record()
-            barrier()
-        ms, _ = reduce_over_ranks(ev0.elapsed_time(ev1), 0.0, world, dev)
+            self.barrier()
+        ms, _ = reduce_over_ranks(ev0.elapsed_time(ev1), 0.0, self.world, self.dev)
         return ms / steps, sie.launch_count() - l0, cs.summary()
 
-    phys_index = local
-    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
-    if vis:
-        try:
-            phys_index = int(vis.split(",")[local])
-        except (ValueError, IndexError):
-            pass
+    def measure(self, name, steps, warmup, want_e2e, want_rdm=False):
+        """Time one workload: device-resident arm (event-timed, stage profile), optional host-I/O e2e arm with the SAME
+        steps/warm-up, optional NEXT-1 call.  Returns a dict of raw measurements (this rank's; times are max over ranks)."""
+        sie, torch, dev = self.sie, self.torch, self.dev
+        specs = workload_specs(name, self.rank)
+        host, devc, t_gen = self.make_inputs(specs, pinned=want_e2e)
+        in_bytes = sum(sum(t.numel() * 8 for t in d.values() if isinstance(t, torch.Tensor)) for d in devc)
+        out_bytes = sum(8 + s.nocc * s.nocc * 8 for s in specs)
+        m = {"name": name, "specs": specs, "in_bytes": in_bytes, "out_bytes": out_bytes, "t_gen": t_gen, "steps": steps, "warmup": warmup}
 
-    # ---- arm 1: inputs resident in HBM
-    step, results, timing, info, ws_bytes = make_step(devc, PROF)
-    ms_step, launches, clocks = timed(step, timing, args.warmup, args.steps, phys_index)
-    stage = timing()
-    E_dev = results()
-    del step, results, timing
-    torch.cuda.empty_cache()
-
-    # ---- FP64 peak probes (live denominators): DMMA, DFMA, smem-fed DMMA
-    probes = {}
-    for kind, name in ((0, "dmma_reg"), (1, "dfma_reg"), (2, "dmma_smem")):
-        best = 0.0
-        for _ in range(3):
-            tf, _ms = sie.sie_dfmp2_probe_fp64(kind, 40000 if kind != 2 else 10000, 2 if kind != 2 else 1)
-            best = max(best, tf)
-        probes[name] = best
-
-    # ---- NEXT-1 (optional): occupied MP2 1-RDM block on the same transformed B, same fused kernel in amplitude mode
-    next1 = None
-    if args.rdm and single:
-        s0, d0 = specs[0], devc[0]
-        plan, nb = sie.sie_dfmp2_plan(s0.nao, s0.nocc, s0.nvir, s0.naux, 0, 0)
-        ws1 = sie.alloc_workspace(nb, dev)
-        sie.sie_dfmp2_transform(plan, ws1, d0["C_occ"], d0["C_vir"], d0["L_packed"], 0, s0.naux)
-        gam = torch.zeros(s0.nocc, s0.nocc, dtype=torch.float64, device=dev)
-        tr = torch.zeros(1, dtype=torch.float64, device=dev)
-        for _ in range(max(1, min(args.warmup, 2))):
-            sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
-        torch.cuda.synchronize()
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = max(1, min(args.steps, 3))
-        ev0.record()
-        for _ in range(reps):
-            sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
-        ev1.record()
-        torch.cuda.synchronize()
-        ms_rdm = ev0.elapsed_time(ev1) / reps
-        f_rdm = alg_flops(s0)["pair_kernel"]  # same contraction count: SYRK of B plus two o^3 products per virtual pair
-        next1 = {"call": "sie_dfmp2_rdm_occ", "ms": ms_rdm, "tflops": f_rdm / (ms_rdm * 1e-3) * 1e-12,
-                 "trace_gamma": float(tr.cpu()[0]), "algorithmic_flops": f_rdm, "includes": "pair kernel (amplitude mode) + reduce"}
-        sie.sie_dfmp2_destroy(plan)
-        del ws1, gam
+        step, results, timing, close, info, ws_bytes = self.make_step(specs, devc, sie.SIE_FLAG_PROFILE)
+        m["ms_step"], m["launches"], m["clocks"] = self.timed(step, timing, warmup, steps)
+        m["stage"] = timing()
+        m["E"] = results()
+        m["info"], m["ws_bytes"] = info, ws_bytes
+        close()
+        del step, results, timing, close
         torch.cuda.empty_cache()
 
-    # ---- arm 2: end to end through the C ABI with host buffers (H2D of every input + D2H of E, G inside the timed region)
-    e2e = None
-    if not args.no_e2e:
-        step, results, timing, _, _ = make_step(host, PROF | sie.SIE_FLAG_HOST_IO)
-        e_warm, e_steps = min(args.warmup, 1), max(1, min(args.steps, 3))
-        ms_e2e, _, _ = timed(step, timing, e_warm, e_steps, phys_index)
-        E_host = results()
-        e2e_stage = timing()
-        del step, results, timing
-        torch.cuda.empty_cache()
+        m["next1"] = None
+        if want_rdm and len(specs) == 1:
+            s0, d0 = specs[0], devc[0]
+            plan, nb = sie.sie_dfmp2_plan(s0.nao, s0.nocc, s0.nvir, s0.naux, 0, 0)
+            ws1 = sie.alloc_workspace(nb, dev)
+            sie.sie_dfmp2_transform(plan, ws1, d0["C_occ"], d0["C_vir"], d0["L_packed"], 0, s0.naux)
+            gam = torch.zeros(s0.nocc, s0.nocc, dtype=torch.float64, device=dev)
+            tr = torch.zeros(1, dtype=torch.float64, device=dev)
+            for _ in range(max(1, min(warmup, 2))):
+                sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
+            torch.cuda.synchronize()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(1, min(steps, 3))
+            ev0.record()
+            for _ in range(reps):
+                sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
+            ev1.record()
+            torch.cuda.synchronize()
+            ms_rdm = ev0.elapsed_time(ev1) / reps
+            f_rdm = alg_flops(s0)["pair_kernel"]  # same contraction count: SYRK of B plus two o^3 products per virtual pair
+            m["next1"] = {"call": "sie_dfmp2_rdm_occ", "ms": ms_rdm, "tflops": f_rdm / (ms_rdm * 1e-3) * 1e-12,
+                          "trace_gamma": float(tr.cpu()[0]), "algorithmic_flops": f_rdm, "includes": "pair kernel (amplitude mode) + reduce"}
+            sie.sie_dfmp2_destroy(plan)
+            del ws1, gam
+            torch.cuda.empty_cache()
 
-    # ---- roofline of the dominant kernel (pair_kernel): algorithmic flops per launch / mean launch duration
-    f_tot = sum(alg_flops(s)["total"] for s in specs)
-    _, f_job = reduce_over_ranks(0.0, f_tot, world, dev)        # units all ranks processed
-    _, n_job = reduce_over_ranks(0.0, float(len(specs)), world, dev)
-    f_pair = sum(alg_flops(s)["pair_kernel"] for s in specs)
-    n_pair = max(1, stage["launch_groups"]["pair"])
-    pair_ms = stage["ms"]["pair"] / n_pair
-    achieved = f_pair / (pair_ms * 1e-3) * 1e-12 if pair_ms > 0 else 0.0
-    peak_probe = max(probes["dmma_reg"], probes["dfma_reg"])
-    peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    peak_rule, rule_src = None, None
-    if os.path.exists(peaks_file):
-        with open(peaks_file) as fh:
-            mp = json.load(fh)
-        # rule of the task: another dtype's measured peak x the guide's nominal ratio (FP64 tensor 45 : bf16 2250 TFLOP/s)
-        peak_rule = float(mp.get("bf16_tflops_sustained", mp.get("bf16_tflops", 0.0))) * 45.0 / 2250.0
-        rule_src = "MEASURED_PEAKS.json bf16_tflops_sustained x 45/2250 (guide's nominal FP64:bf16 tensor ratio)"
+        m["e2e"] = None
+        if want_e2e:
+            step, results, timing, close, _, _ = self.make_step(specs, host, sie.SIE_FLAG_PROFILE | sie.SIE_FLAG_HOST_IO)
+            ms_e2e, _, _ = self.timed(step, timing, warmup, steps)
+            E_host = results()
+            close()
+            del step, results, timing, close
+            m["e2e"] = {"ms": ms_e2e, "E": E_host}
+        del host, devc
+        torch.cuda.empty_cache()
+        return m
+
+    def summarize(self, m):
+        """Derived figures of one measured workload: whole-step rate, pair-kernel roofline, transform fractions."""
+        specs, stage, steps = m["specs"], m["stage"], m["steps"]
+        f_tot = sum(alg_flops(s)["total"] for s in specs)
+        _, f_job = reduce_over_ranks(0.0, f_tot, self.world, self.dev)  # units all ranks processed
+        _, n_job = reduce_over_ranks(0.0, float(len(specs)), self.world, self.dev)
+        f_pair = sum(alg_flops(s)["pair_kernel"] for s in specs)
+        n_pair = max(1, stage["launch_groups"]["pair"])
+        pair_ms = stage["ms"]["pair"] / n_pair
+        achieved = f_pair / (pair_ms * 1e-3) * 1e-12 if pair_ms > 0 else 0.0
+        peak = self.peak
+        traffic, traffic_src = ncu_pair_traffic(m["name"])
+        roofline = {
+            "kernel": "pair_kernel", "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "frac": achieved / peak if peak else None, "launches": n_pair, "ms_per_launch": pair_ms,
+            "algorithmic_flops_per_launch": f_pair, "traffic": traffic, "traffic_source": traffic_src,
+        }
+        if len(specs) == 1:
+            fx = exec_pair_flops(specs[0], m["info"])
+            roofline["executed"] = fx / (pair_ms * 1e-3) * 1e-12 if pair_ms > 0 else None
+            roofline["executed_frac"] = roofline["executed"] / peak if peak and roofline["executed"] else None
+        # transform stage (A1 + A2 incl. coefficient copies and, where it still exists, the unpack): both fractions (SURVEY.md §8(d)).
+        # In a batch the per-cluster transforms overlap on side streams, so the stage SUM is an upper bound of their wall time.
+        tr_ms = (stage["ms"]["unpack"] + stage["ms"]["A1_gemm"] + stage["ms"]["A2_gemm"] + stage["ms"]["coeff_transpose"]) / max(1, steps)
+        f_tr = sum(alg_flops(s)["A1"] + alg_flops(s)["A2"] for s in specs)
+        b_tr = sum(8.0 * s.naux * s.npair + 8.0 * s.nocc * s.nvir * s.naux for s in specs)
+        hbm_peak = measured_peaks().get("hbm_gbs")
+        transform = {
+            "ms_per_step": tr_ms, "tflops": f_tr / (tr_ms * 1e-3) * 1e-12 if tr_ms > 0 else None,
+            "algorithmic_gbs": b_tr / (tr_ms * 1e-3) * 1e-9 if tr_ms > 0 else None, "hbm_peak_gbs": hbm_peak,
+            "frac_hbm": (b_tr / (tr_ms * 1e-3) * 1e-9 / hbm_peak) if (tr_ms > 0 and hbm_peak) else None,
+            "frac_fp64": (f_tr / (tr_ms * 1e-3) * 1e-12 / peak) if (tr_ms > 0 and peak) else None,
+        }
+        return {"f_tot": f_tot, "f_job": f_job, "n_job": n_job, "value": f_job / (m["ms_step"] * 1e-3) * 1e-12,
+                "clusters_per_s": n_job / (m["ms_step"] * 1e-3), "roofline": roofline, "transform": transform}
+
+    def sub_object(self, name, steps, warmup):
+        """A time-boxed secondary workload measured in the same process with the same event timing (no e2e arm)."""
+        m = self.measure(name, steps, warmup, want_e2e=False)
+        z = self.summarize(m)
+        s0 = m["specs"][0]
+        out = {"workload": name, "clusters": len(m["specs"]), "steps": steps, "warmup": warmup, "ms_per_step": m["ms_step"],
+               "tflops": z["value"], "clusters_per_s": z["clusters_per_s"], "pair_ms": z["roofline"]["ms_per_launch"],
+               "pair_tflops": z["roofline"]["achieved"], "pair_frac": z["roofline"]["frac"],
+               "transform_ms": z["transform"]["ms_per_step"], "transform_tflops": z["transform"]["tflops"],
+               "transform_frac": z["transform"]["frac_fp64"], "gpu_launches": m["launches"],
+               "sm_mhz": m["clocks"].get("sm_mhz"), "reasons": m["clocks"].get("reasons"),
+               "E_frag": m["E"][:2], "stage_ms_per_step": {k: v / max(1, steps) for k, v in m["stage"]["ms"].items()}}
+        if len(m["specs"]) == 1:
+            out.update({"nocc": s0.nocc, "nvir": s0.nvir, "nao": s0.nao, "naux": s0.naux})
+        return out
+
+
+def measured_peaks() -> dict:
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return json.load(fh)
+    except (OSError, ValueError):
+        return {}
+
+
+def run_gpu(args) -> None:
+    gb = GpuBench()
+    m = gb.measure(args.workload, args.steps, args.warmup, want_e2e=not args.no_e2e, want_rdm=args.rdm)
+    gb.probe_peak()
+    z = gb.summarize(m)
+    specs, stage, clocks = m["specs"], m["stage"], m["clocks"]
+    roofline = z["roofline"]
+    mp = measured_peaks()
     sm_mhz = clocks.get("sm_mhz") or 0.0
-    roofline = {
-        "kernel": "pair_kernel", "bound": "tensor", "achieved": achieved, "peak": peak_probe, "unit": "TFLOP/s",
-        "frac": achieved / peak_probe if peak_probe else None,
+    roofline.update({
         "peak_source": "live sie_dfmp2_probe_fp64: register-resident mma.sync.m8n8k4.f64 / DFMA issue-rate loop on all SMs "
                        "(MEASURED_PEAKS.json has no FP64 entry); the larger of the two",
-        "probes_tflops": probes,
-        "peak_rule": peak_rule, "peak_rule_source": rule_src,
+        "probes_tflops": gb.probes,
+        # rule of the task: another dtype's measured peak x the guide's nominal ratio (FP64 tensor 45 : bf16 2250 TFLOP/s)
+        "peak_rule": float(mp.get("bf16_tflops_sustained", mp.get("bf16_tflops", 0.0))) * 45.0 / 2250.0 if mp else None,
+        "peak_rule_source": "MEASURED_PEAKS.json bf16_tflops_sustained x 45/2250 (guide's nominal FP64:bf16 tensor ratio)" if mp else None,
         "peak_nominal_at_clock": 148 * 128 * sm_mhz * 1e6 * 1e-12 if sm_mhz else None,  # 64 DFMA/clk/SM x 2 flop
-        "launches": n_pair, "ms_per_launch": pair_ms,
-        "algorithmic_flops_per_launch": f_pair,
-        "traffic": NCU_PAIR_TRAFFIC_BYTES.get(args.workload),
-    }
-    if single:
-        fx = exec_pair_flops(specs[0], info)
-        roofline["executed"] = fx / (pair_ms * 1e-3) * 1e-12 if pair_ms > 0 else None
-        roofline["executed_frac"] = roofline["executed"] / peak_probe if peak_probe and roofline["executed"] else None
-    # transform stage (A1+A2, incl. unpack): both fractions, SURVEY.md §8(d)
-    tr_ms = (stage["ms"]["unpack"] + stage["ms"]["A1_gemm"] + stage["ms"]["A2_gemm"] + stage["ms"]["coeff_transpose"]) / max(1, args.steps)
-    f_tr = sum(alg_flops(s)["A1"] + alg_flops(s)["A2"] for s in specs)
-    b_tr = sum(8.0 * s.naux * s.npair + 8.0 * s.nocc * s.nvir * s.naux for s in specs)
-    hbm_peak = None
-    if os.path.exists(peaks_file):
-        hbm_peak = float(mp.get("hbm_gbs", 0.0)) or None
-    transform = {
-        "ms_per_step": tr_ms, "tflops": f_tr / (tr_ms * 1e-3) * 1e-12 if tr_ms > 0 else None,
-        "algorithmic_gbs": b_tr / (tr_ms * 1e-3) * 1e-9 if tr_ms > 0 else None, "hbm_peak_gbs": hbm_peak,
-        "frac_hbm": (b_tr / (tr_ms * 1e-3) * 1e-9 / hbm_peak) if (tr_ms > 0 and hbm_peak) else None,
-        "frac_fp64": (f_tr / (tr_ms * 1e-3) * 1e-12 / peak_probe) if (tr_ms > 0 and peak_probe) else None,
-    }
+    })
+
+    # ---- the other halves of the metric, time-boxed, same process / same timing: clusters/s of the 96-cluster batch
+    #      (config 2) and the roofline fraction at each resident point of the size sweep (config 4)
+    batch, sweep = None, None
+    if args.extras and gb.world == 1 and args.workload == "config3":
+        k, w = max(1, min(args.steps, 3)), 3
+        batch = gb.sub_object("config2", k, w)
+        sweep = [gb.sub_object(f"config4:{i}", k, w) for i in range(3)]  # v = 256, 512, 1024 (v = 2048: --streamed)
 
     # ---- CPU oracle beside it (rank 0, N = 1 only): bounded sample, extrapolated
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu:
+    if gb.rank == 0 and gb.world == 1 and not args.no_cpu:
         secs, spent, desc, cores = oracle_workload_seconds(specs)
-        cpu = {"value": f_tot / secs * 1e-12, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+        cpu = {"value": z["f_tot"] / secs * 1e-12, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                "extrapolated_s_per_step": secs, "measured_s": spent}
 
-    if rank == 0:
-        value = f_job / (ms_step * 1e-3) * 1e-12
+    if gb.rank == 0:
+        l2 = "inputs larger than L2 (no flush needed)" if m["in_bytes"] > (126 << 20) else "inputs smaller than L2; L2 not flushed"
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": workload_config(args.workload, specs, "inputs larger than L2 (no flush needed)" if in_bytes > (126 << 20) else "inputs smaller than L2; L2 not flushed"),
-            "clusters_per_s": n_job / (ms_step * 1e-3),
-            "E_frag": E_dev if len(E_dev) <= 4 else E_dev[:4],
+            "metric": METRIC, "value": z["value"], "unit": UNIT, "n_gpus": gb.world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": m["ms_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(args.workload, specs, l2),
+            "clusters_per_s": z["clusters_per_s"],
+            "E_frag": m["E"] if len(m["E"]) <= 4 else m["E"][:4],
             "stage_ms_per_step": {k: v / max(1, args.steps) for k, v in stage["ms"].items()},
-            "roofline": roofline, "transform": transform, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": launches,
-            "workspace_bytes": ws_bytes, "input_gen_s": t_gen,
+            "roofline": roofline, "transform": z["transform"], "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": m["launches"],
+            "workspace_bytes": m["ws_bytes"], "input_gen_s": m["t_gen"],
         }
-        if next1 is not None:
-            next1["frac_of_fp64_peak"] = next1["tflops"] / peak_probe if peak_probe else None
-            line["next1_rdm_occ"] = next1
-        if e2e is None and not args.no_e2e:
-            e2e = {"value": f_job / (ms_e2e * 1e-3) * 1e-12, "unit": UNIT, "ms_per_step": ms_e2e,
-                   "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes, "steps": e_steps,
-                   "h2d_gbs": in_bytes / (ms_e2e * 1e-3) * 1e-9,
-                   "same_result_as_device_arm": bool(all(abs(a - b) <= 1e-12 * abs(a) for a, b in zip(E_dev, E_host)))}
+        if m["next1"] is not None:
+            m["next1"]["frac_of_fp64_peak"] = m["next1"]["tflops"] / gb.peak if gb.peak else None
+            line["next1_rdm_occ"] = m["next1"]
+        if batch is not None:
+            line["batch"] = batch
+            line["sweep"] = sweep
+        e2e = None
+        if m["e2e"] is not None:
+            ms_e2e = m["e2e"]["ms"]
+            e2e = {"value": z["f_job"] / (ms_e2e * 1e-3) * 1e-12, "unit": UNIT, "ms_per_step": ms_e2e,
+                   "h2d_bytes_per_step": m["in_bytes"], "d2h_bytes_per_step": m["out_bytes"], "steps": args.steps, "warmup": args.warmup,
+                   "h2d_gbs": m["in_bytes"] / (ms_e2e * 1e-3) * 1e-9,
+                   "same_result_as_device_arm": bool(all(abs(a - b) <= 1e-12 * abs(a) for a, b in zip(m["E"], m["e2e"]["E"])))}
         line["e2e"] = e2e
         print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    if gb.world > 1:
+        gb.dist.destroy_process_group()
 
 
 # ------------------------------------------------------------------------------------------------ streamed sweep point
@@ -572,6 +649,8 @@ def main() -> None:
     ap.add_argument("--impl", default="sie", choices=["sie", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end arm")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle leg")
+    ap.add_argument("--no-extras", dest="extras", action="store_false",
+                    help="skip the time-boxed config-2 batch and config-4 sweep sub-objects of the default config-3 line")
     ap.add_argument("--rdm", action="store_true", help="also time sie_dfmp2_rdm_occ (NEXT-1: occupied MP2 1-RDM block) on the same B")
     ap.add_argument("--streamed", action="store_true", help="feed the packed integrals in aux blocks generated on the fly "
                                                              "(sweep points that do not fit in HBM; not a bench line)")

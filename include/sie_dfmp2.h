@@ -130,6 +130,15 @@ typedef struct {
 int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes,
                     size_t* needed, unsigned flags, void* cuda_stream);
 
+/*
+ * Forgets which aux rows have been transformed (host-side state only; enqueues nothing), so the same plan can run
+ * another cluster of the same shape — or the same one again — with the same or another workspace:
+ * plan -> [transform... -> energy...] -> reset -> [transform... -> energy...] -> destroy.
+ * Work already enqueued is not affected; the caller orders reuse of the workspace by using one stream.
+ * A transform into a different workspace than the rows covered so far returns SIE_ESTATE unless reset first.
+ */
+int sie_dfmp2_plan_reset(sie_dfmp2_plan_t plan);
+
 /* Frees the host-side plan (never touches device memory). NULL is allowed. */
 int sie_dfmp2_destroy(sie_dfmp2_plan_t plan);
 

@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     sie_dfmp2_rdm_occ,
     sie_dfmp2_plan,
     sie_dfmp2_plan_info,
+    sie_dfmp2_plan_reset,
     sie_dfmp2_plan_timing,
     sie_dfmp2_batch_timing,
     sie_dfmp2_probe_fp64,

@@ -24,6 +24,7 @@ EXPORTS = (
     "sie_dfmp2_energy",
     "sie_dfmp2_rdm_occ",
     "sie_dfmp2_batch",
+    "sie_dfmp2_plan_reset",
     "sie_dfmp2_destroy",
     "sie_dfmp2_strerror",
     "sie_dfmp2_last_cuda_error",
@@ -85,6 +86,8 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_rdm_occ.restype = ci
         L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
         L.sie_dfmp2_batch.restype = ci
+        L.sie_dfmp2_plan_reset.argtypes = [vp]
+        L.sie_dfmp2_plan_reset.restype = ci
         L.sie_dfmp2_destroy.argtypes = [vp]
         L.sie_dfmp2_destroy.restype = ci
         L.sie_dfmp2_strerror.argtypes = [ci]
@@ -167,6 +170,10 @@ def sie_dfmp2_energy(plan: int, workspace: torch.Tensor, e_occ, e_vir, P_frag, E
             _ptr(E_out, host, "E_out"), _ptr(G_out, host, "G_out"), _stream_ptr(stream)),
         "sie_dfmp2_energy",
     )
+
+
+def sie_dfmp2_plan_reset(plan: int) -> None:
+    _check(_lib().sie_dfmp2_plan_reset(plan), "sie_dfmp2_plan_reset")
 
 
 def sie_dfmp2_destroy(plan: Optional[int]) -> None:
@@ -290,6 +297,10 @@ class ClusterSolver:
 
     def timing(self) -> dict:
         return sie_dfmp2_plan_timing(self.plan)
+
+    def reset(self) -> None:
+        """Forget the transformed rows: the plan and workspace can take the next cluster of the same shape."""
+        sie_dfmp2_plan_reset(self.plan)
 
     def close(self) -> None:
         sie_dfmp2_destroy(self.plan)

@@ -44,17 +44,28 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 static EncodeTiledFn get_encode_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // function-local static: initialised once, thread-safe (C++11); the entry point is process-wide, not per device
+    static const EncodeTiledFn fn = []() -> EncodeTiledFn {
         void* p = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
             q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(p);
-    }
+            return reinterpret_cast<EncodeTiledFn>(p);
+        return nullptr;
+    }();
     return fn;
+}
+
+int ensure_smem_attr(const void* kernel, int bytes, SmemAttrOnce& once) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return set_cuda_error(e);
+    const bool tracked = dev >= 0 && dev < 64;
+    if (tracked && (__atomic_load_n(&once.done, __ATOMIC_ACQUIRE) >> dev & 1ull)) return SIE_OK;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return set_cuda_error(e);
+    if (tracked) __atomic_fetch_or(&once.done, 1ull << dev, __ATOMIC_RELEASE);
+    return SIE_OK;
 }
 
 int make_tensor_map_3d(CUtensorMap* out, const double* base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t stride1_bytes,
@@ -79,31 +90,38 @@ int make_tensor_map_3d(CUtensorMap* out, const double* base, uint64_t d0, uint64
     return SIE_OK;
 }
 
+// Facts of the CURRENT device (cudaGetDevice of the calling thread), cached per device ordinal in atomics:
+// a process may drive several GPUs and several host threads may plan concurrently.
+static std::atomic<int> g_dev_sms[64];    // 0 = not queried yet
+static std::atomic<int> g_dev_major[64];  // 0 = not queried yet
+
 static int query_num_sms() {
-    static int sms = -1;
-    if (sms < 0) {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-            sms = n;
-        else {
-            (void)cudaGetLastError();
-            return 148;  // planning without a device (CPU-only host): B200 value
-        }
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 148;  // planning without a device (CPU-only host): B200 value
     }
-    return sms;
+    const bool tracked = dev >= 0 && dev < 64;
+    if (tracked && (n = g_dev_sms[dev].load(std::memory_order_relaxed)) > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+        (void)cudaGetLastError();
+        return 148;
+    }
+    if (tracked) g_dev_sms[dev].store(n, std::memory_order_relaxed);
+    return n;
 }
 
 static int check_device() {
-    static int ok = -1;
-    if (ok < 0) {
-        int dev = 0, major = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    int dev = 0, major = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return set_cuda_error(e);
+    const bool tracked = dev >= 0 && dev < 64;
+    if (!tracked || (major = g_dev_major[dev].load(std::memory_order_relaxed)) == 0) {
+        e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
         if (e != cudaSuccess) return set_cuda_error(e);
-        ok = (major == 10) ? 1 : 0;
+        if (tracked) g_dev_major[dev].store(major, std::memory_order_relaxed);
     }
-    return ok == 1 ? SIE_OK : SIE_EUNSUPPORTED;
+    return major == 10 ? SIE_OK : SIE_EUNSUPPORTED;
 }
 
 }  // namespace sie
@@ -348,7 +366,14 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
     CUtensorMap mapCo, mapCv;
     SIE_TRY(make_tensor_map_3d(&mapCo, sc.CoT, nao, o, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * o, 8, tm1, 1));
     SIE_TRY(make_tensor_map_3d(&mapCv, sc.CvT, nao, v, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * v, 8, tm2, 1));
-    if (host_L) SIE_TRY(ensure_copy_pipeline(pipe_owner));
+    if (host_L) {
+        // the staging copies of this call must not start before earlier work on `st` that owns the workspace: ONE fork per
+        // call; after that only the per-buffer ready/consumed events order the ring, so the H2D copy of sub-block n+1 runs
+        // under the unpack/A1/A2 of sub-block n
+        SIE_TRY(ensure_copy_pipeline(pipe_owner));
+        SIE_CUDA(cudaEventRecord(pipe_owner.ev_fork, st));
+        SIE_CUDA(cudaStreamWaitEvent(pipe_owner.copy_stream, pipe_owner.ev_fork, 0));
+    }
     for (int q0 = p0; q0 < p1; q0 += p.pblk) {
         const int q1 = std::min(p1, q0 + p.pblk), pb = q1 - q0;
         const double* Lq = L + (size_t)(q0 - p0) * p.npair;
@@ -358,8 +383,6 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
             const int buf = po.stage_turn & 1;
             po.stage_turn++;
             unsigned char* dst = sc.stage + (size_t)buf * sc.stage_buf_bytes;
-            SIE_CUDA(cudaEventRecord(po.ev_fork, st));  // staging must not start before earlier work on `st` that owns the workspace
-            SIE_CUDA(cudaStreamWaitEvent(po.copy_stream, po.ev_fork, 0));
             SIE_CUDA(cudaStreamWaitEvent(po.copy_stream, po.ev_consumed[buf], 0));
             SIE_CUDA(cudaMemcpyAsync(dst, Lq, (size_t)pb * p.npair * 8, cudaMemcpyHostToDevice, po.copy_stream));
             SIE_CUDA(cudaEventRecord(po.ev_ready[buf], po.copy_stream));
@@ -524,6 +547,9 @@ int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_
     if (p0 < 0 || p1 > p.naux || p0 >= p1) return SIE_EINVAL;
     if (reinterpret_cast<uintptr_t>(workspace) & 255) return SIE_EINVAL;
     SIE_TRY(check_device());
+    // B of the rows covered so far lives in the workspace they were transformed into: a different workspace mid-way
+    // would leave rows missing (sie_dfmp2_plan_reset starts over)
+    if (!p.covered.empty() && p.c_ready_ws != workspace) return SIE_ESTATE;
     for (auto& iv : p.covered)
         if (p0 < iv.second && iv.first < p1) return SIE_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -864,6 +890,15 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
     } catch (const std::bad_alloc&) {
         return SIE_ENOMEM;
     }
+}
+
+int sie_dfmp2_plan_reset(sie_dfmp2_plan_t plan) {
+    if (!plan) return SIE_EINVAL;
+    plan->covered.clear();
+    plan->covered_rows = 0;
+    plan->c_ready_ws = nullptr;
+    plan->dC_occ = plan->dC_vir = nullptr;
+    return SIE_OK;
 }
 
 int sie_dfmp2_destroy(sie_dfmp2_plan_t plan) {

@@ -76,6 +76,12 @@ __device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* m
         "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
         : "memory");
 }
+// A tensor map that lives in global memory (not a __grid_constant__ kernel parameter) was written through the generic
+// proxy (here: a cudaMemcpyAsync into the workspace); before the first cp.async.bulk.tensor that reads it through the
+// tensormap proxy the issuing thread must acquire it, or a descriptor-cache hit may serve stale contents of that address.
+__device__ __forceinline__ void tma_acquire_desc(const CUtensorMap* map) {
+    asm volatile("fence.proxy.tensormap::generic.acquire.sys [%0], 128;" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
+}
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
 }
@@ -89,6 +95,12 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 // host side
 // ------------------------------------------------------------------------------------------------
 void note_launch();                      // counts kernel launches (api.cu)
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a per-device setting: `done` is a per-kernel bit mask over device
+// ordinals (api.cu); devices >= 64 set the attribute on every launch.  Thread-safe (atomic mask, idempotent call).
+struct SmemAttrOnce {
+    unsigned long long done = 0;
+};
+int ensure_smem_attr(const void* kernel, int bytes, SmemAttrOnce& once);
 int set_cuda_error(cudaError_t e);       // records the text, returns SIE_ECUDA
 int set_cuda_error_text(const char* s);  // records the text, returns SIE_ECUDA
 

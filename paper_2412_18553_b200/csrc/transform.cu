@@ -140,12 +140,9 @@ static int launch_gemm_cfg(const CUtensorMap& mapA, const CUtensorMap& mapB, int
                            long long inner_pad, int kblocks, const GemmOut& out, int num_sms, cudaStream_t st) {
     const size_t smem = (size_t)Cfg::STAGES * Cfg::STAGE_BYTES + 2 * Cfg::STAGES * sizeof(uint64_t) + 128;
     auto kern = gemm_tn_kernel<Cfg>;
-    static bool attr_set = false;  // per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return set_cuda_error(e);
-        attr_set = true;
-    }
+    static SmemAttrOnce once;  // per instantiation, per device inside
+    const int rc = ensure_smem_attr(reinterpret_cast<const void*>(kern), (int)smem, once);
+    if (rc != SIE_OK) return rc;
     const long long ntiles = (long long)m_tiles * n_tiles;
     if (ntiles <= 0) return SIE_OK;
     const int grid = (int)(ntiles < num_sms ? ntiles : num_sms);

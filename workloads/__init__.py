@@ -10,4 +10,5 @@ from .gen import (  # noqa: F401
     config_specs,
     make_cluster,
     npair,
+    virtual_subset,
 )

@@ -23,7 +23,7 @@ from typing import List, Optional
 import numpy as np
 
 # stream ids inside SeedSequence([config_id, cluster_id, stream_id])
-_S_C, _S_EOCC, _S_EVIR, _S_Q, _S_NOCC = 1, 2, 3, 4, 5
+_S_C, _S_EOCC, _S_EVIR, _S_Q, _S_NOCC, _S_SUBSET = 1, 2, 3, 4, 5, 6
 _S_L0 = 100  # aux index P uses stream 100 + P
 
 
@@ -109,6 +109,17 @@ class ClusterInputs:
 
     def L_packed(self, threads: int = 1) -> np.ndarray:
         return self.L_block(0, self.spec.naux, threads=threads)
+
+
+def virtual_subset(spec: ClusterSpec, k: int) -> np.ndarray:
+    """Sorted, seeded choice of ``k`` of the ``nvir`` virtual columns, always containing the first and the last one.
+
+    Used by the "dense aux x k dense virtuals" full-size parity case: C_vir is zeroed outside these
+    columns, so the CPU side only needs the compressed problem while the GPU runs the full-size launch."""
+    assert 2 <= k <= spec.nvir
+    r = _rng(spec, _S_SUBSET)
+    inner = r.choice(np.arange(1, spec.nvir - 1), size=k - 2, replace=False)
+    return np.sort(np.concatenate([[0, spec.nvir - 1], inner])).astype(np.int64)
 
 
 def make_cluster(spec: ClusterSpec) -> ClusterInputs:
