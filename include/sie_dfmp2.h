@@ -62,7 +62,7 @@ enum {
 
 /*
  * 1. sie_dfmp2_plan — host only.  Validates the sizes, chooses tile configurations and the internal aux
- *    sub-block, and reports the device workspace (bytes, 256-byte aligned base required) the caller must
+ *    sub-block (the rows of the half-transformed intermediate H that exist at once; at most 2 GB), and reports the device workspace (bytes, 256-byte aligned base required) the caller must
  *    pass to transform/energy.  The workspace holds B[a][i][P] between transform and energy.
  *      nao >= nocc + nvir, nocc >= 1, nvir >= 1, naux >= 1; aux_block = rows of (P|mu nu) processed per
  *      internal step (0 = auto).  nocc > 128 silently selects the reference kernels.
@@ -109,9 +109,9 @@ int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_oc
  *    static, cost-balanced list of (cluster, tile) work items, then one reduction launch (step A7).
  *      clusters: HOST array of descriptors (pointers device or host per SIE_FLAG_HOST_IO).
  *      workspace_bytes == 0 or workspace == NULL: query only, *needed receives the required size.
- *    With device pointers the per-cluster transforms run on up to 4 internal side streams that are forked from
- *    and joined back into `cuda_stream` with events (all work is ordered after what was enqueued on `cuda_stream`
- *    before the call, and the results are ready when `cuda_stream` reaches the end of the call's work).
+ *    With device pointers the transforms of ALL clusters run as one grouped launch per stage (coefficient transposes,
+ *    A1 on the packed integrals, A2) and everything is enqueued on `cuda_stream`; with host pointers the clusters'
+ *    integrals pass through one staging ring on an internal copy stream, cluster by cluster.
  *    Errors: SIE_EINVAL (sizes, null required pointers, misaligned workspace), SIE_ENOMEM (workspace too small;
  *    *needed is set), SIE_EGAP (SIE_FLAG_VALIDATE), SIE_ECUDA.  Outputs are untouched on SIE_EINVAL/SIE_ENOMEM.
  */
@@ -162,7 +162,7 @@ int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n);
 /*
  * Stage timing (plans / batches created with SIE_FLAG_PROFILE; SIE_ESTATE otherwise).  Synchronises on the
  * recorded events, sums the device time of every launch group enqueued since the last query, then clears.
- *   ms[0..7):  0 coefficient transposes  1 unpack (packed -> square)  2 A1 GEMM  3 A2 GEMM  4 fused pair kernel
+ *   ms[0..7):  0 coefficient transposes  1 unused (always 0: A1 reads the packed triangle directly)  2 A1 GEMM  3 A2 GEMM  4 fused pair kernel
  *              5 reduce/trace  6 reference kernels          (milliseconds, HOST array of n doubles)
  *   ms[7..14): the number of launch groups summed into each of the seven entries above.
  * sie_dfmp2_batch_timing reports the calling thread's last sie_dfmp2_batch call.

@@ -197,12 +197,12 @@ struct sie_dfmp2_plan_s {
     int nao = 0, o = 0, v = 0, naux = 0;
     unsigned flags = 0;
     bool ref = false;
-    int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, t8 = 8, nblk = 0, pblk = 0, ncta = 0, kp = 1, num_sms = 148;
+    int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, t8 = 8, nblk = 0, pblk = 0, cblk = 0, max_jobs = 0, ncta = 0, kp = 1, num_sms = 148;
     size_t npair = 0;
     std::vector<PairTile> tiles;  // cluster field = 0; rewritten when used inside a batch
     double tile_cost = 0;         // relative cost of one tile (for batch ordering)
     // workspace offsets (bytes)
-    size_t off_B = 0, off_CoT = 0, off_CvT = 0, off_Lfull = 0, off_H = 0, off_gpart = 0, off_desc = 0, off_tiles = 0, off_rc = 0,
+    size_t off_B = 0, off_CoT = 0, off_CvT = 0, off_jobs = 0, off_H = 0, off_gpart = 0, off_desc = 0, off_tiles = 0, off_rc = 0,
            off_stage = 0, off_io = 0, off_refH = 0, off_refVj = 0, off_refG = 0, total = 0;
     size_t gpart_bytes = 0, stage_buf_bytes = 0;
     // io sub-offsets (doubles, relative to off_io)
@@ -243,7 +243,9 @@ void build_tiles(int nblk, std::vector<PairTile>& out) {
     }
 }
 
-int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags, bool carve_shared) {
+enum { CARVE_NONE = 0, CARVE_MEMBER = 1, CARVE_ALL = 2 };  // what plan_init lays out beside B and the partial-G slots
+
+int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags, int carve) {
     if (nao < 1 || nocc < 1 || nvir < 1 || naux < 1 || aux_block < 0) return SIE_EINVAL;
     if ((long long)nocc + nvir > nao) return SIE_EINVAL;
     if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE)) return SIE_EINVAL;
@@ -259,21 +261,22 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
     p.nao_ld = (int)align_up((size_t)nao, 8);
     p.naux_ld = (int)align_up((size_t)naux, 8);
     p.o8 = (int)align_up((size_t)nocc, 8);
-    // internal aux sub-block
-    if (aux_block > 0) {
-        p.pblk = std::min(aux_block, naux);
-    } else if (p.ref) {
-        p.pblk = std::min(naux, 64);
+    // internal aux sub-block = the rows of H[i][P][nu] that exist at once between A1 and A2
+    if (p.ref) {
+        p.pblk = std::min(naux, aux_block > 0 ? aux_block : 64);
+        p.cblk = p.pblk;
     } else {
-        // aux sub-block: enough 128-column tiles of A1 for ~8 full waves of the persistent GEMM (tail < 1/8 wave),
-        // at most 128 aux rows and at most 2 GB for the unpacked square block
-        const int nvb = (nao + 127) / 128;
-        int pb = (8 * p.num_sms + nvb - 1) / nvb;
-        const size_t per_p = (size_t)nao * p.nao_ld * 8;
-        const int cap = (int)std::max<size_t>(8, ((size_t)2048 << 20) / per_p);
-        pb = std::max(8, std::min(std::min(pb, 128), cap));
-        pb = (pb + 7) / 8 * 8;
-        p.pblk = std::min(pb, naux);
+        // at most 2 GB of H, and flat column indices (P, nu) and (i, P) of the two GEMMs below 2^31; each sub-block is ONE
+        // grouped launch per stage, so there is no reason to make it smaller than that
+        const size_t per_p = (size_t)nocc * p.nao_ld * 8;
+        long long pb = std::max<long long>(8, (long long)(((size_t)2 << 30) / per_p));
+        pb = std::min<long long>(pb, (long long)0x7fffffff / std::max(nao, nocc) - 1);
+        if (aux_block > 0) pb = std::min<long long>(pb, aux_block);
+        if (pb < naux) pb = std::max<long long>(8, pb / 8 * 8);
+        p.pblk = (int)std::min<long long>(pb, naux);
+        // HOST_IO: rows of packed (P|mu nu) per staging buffer (512 MB each, two of them)
+        long long cb = std::max<long long>(8, (long long)(((size_t)512 << 20) / (p.npair * 8)) / 8 * 8);
+        p.cblk = (int)std::min<long long>(cb, p.pblk);
     }
     if (!p.ref) {
         // pair tiling: ta whole virtual blocks (ta*o <= 128 rows of B, o itself is never padded) per tile edge
@@ -295,12 +298,19 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
         p.off_gpart = c.take(p.gpart_bytes);
     else
         p.off_refG = c.take((size_t)nocc * nocc * 8);
-    if (carve_shared) {
+    // job descriptors of one transform call: one A1 job per staged chunk (HOST_IO) or per sub-block, one A2 job per sub-block
+    p.max_jobs = (naux + p.pblk - 1) / p.pblk + (naux + p.cblk - 1) / p.cblk + 8;
+    if (carve == CARVE_MEMBER && !p.ref) {  // member of a device-pointer batch: private coefficient copies and H
+        p.off_CoT = c.take((size_t)nocc * p.nao_ld * 8);
+        p.off_CvT = c.take((size_t)nvir * p.nao_ld * 8);
+        p.off_H = c.take((size_t)nocc * p.pblk * p.nao_ld * 8);
+    }
+    if (carve == CARVE_ALL) {
         if (!p.ref) {
             p.off_CoT = c.take((size_t)nocc * p.nao_ld * 8);
             p.off_CvT = c.take((size_t)nvir * p.nao_ld * 8);
-            p.off_Lfull = c.take((size_t)p.pblk * nao * p.nao_ld * 8);
             p.off_H = c.take((size_t)nocc * p.pblk * p.nao_ld * 8);
+            p.off_jobs = c.take((size_t)p.max_jobs * sizeof(XJob) + 2 * sizeof(TJob));
             p.off_desc = c.take(sizeof(PairCluster));
             p.off_tiles = c.take(p.tiles.size() * sizeof(PairTile) + 256);  // + the round-gate counter behind the list
         } else {
@@ -309,7 +319,7 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
         }
         p.off_rc = c.take(sizeof(ReduceCluster));
         if (flags & SIE_FLAG_HOST_IO) {
-            p.stage_buf_bytes = align_up((size_t)p.pblk * p.npair * 8, 256);
+            p.stage_buf_bytes = align_up((size_t)p.cblk * p.npair * 8, 256);
             p.off_stage = c.take(2 * p.stage_buf_bytes);
             size_t d = 0;
             p.io_Cocc = d, d += (size_t)nao * nocc;
@@ -338,13 +348,77 @@ int ensure_copy_pipeline(sie_dfmp2_plan_s& p) {
     return SIE_OK;
 }
 
-struct Scratch {  // shared transform scratch (device pointers)
-    double *CoT, *CvT, *Lfull, *H, *refH;
+struct Scratch {  // transform scratch of one cluster (device pointers)
+    double *CoT, *CvT, *H, *refH;
+    unsigned char* jobs;   // arena of max_jobs XJob + 2 TJob descriptors
     unsigned char* stage;  // HOST_IO: 2 staging buffers
     size_t stage_buf_bytes;
 };
 
-// Transform of aux rows [p0,p1) into Bmat ([v][o][naux_ld]).  L points at row p0 (device, or host when host_L).
+// ---- job descriptors of the grouped transform GEMMs (transform.cu)
+// A1 on `np` packed rows starting at Lq: H[i][P][nu] for P in [h0, h0+np) of an H sub-block that holds pbH rows
+int make_a1_job(XJob& J, const sie_dfmp2_plan_s& p, const double* CoT, const double* Lq, int np, double* H, int h0, int pbH) {
+    std::memset(&J, 0, sizeof J);
+    const int m8 = p.o8 / 8;
+    SIE_TRY(make_tensor_map_3d(&J.mapA, CoT, p.nao, p.o, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * p.o, 8, 8 * m8, 1));
+    J.Lp = Lq;
+    J.npair = (long long)p.npair;
+    J.nao = p.nao;
+    J.n_total = (long long)np * p.nao;
+    J.M = p.o;
+    J.m8 = m8;
+    J.m_tiles = 1;
+    J.n_tiles = (int)((J.n_total + 127) / 128);
+    J.kblocks = (p.nao + 7) / 8;
+    J.out.base = H + (size_t)h0 * p.nao_ld;
+    J.out.ld_m = (long long)pbH * p.nao_ld;
+    J.out.M = p.o;
+    J.out.inner = p.nao;
+    J.out.valid_inner = p.nao;
+    J.out.stride_outer = p.nao_ld;
+    J.out.n_lin_total = J.n_total;
+    return SIE_OK;
+}
+// A2 on an H sub-block of pb aux rows starting at aux index q0: B[a][i][q0+P] = sum_nu CvT[a][nu] * H[(i,P)][nu]
+int make_a2_job(XJob& J, const sie_dfmp2_plan_s& p, const double* CvT, const double* H, int pb, double* Bmat, int q0) {
+    std::memset(&J, 0, sizeof J);
+    const int m_tiles = (p.v + 127) / 128;
+    const int m8 = ((p.v + m_tiles - 1) / m_tiles + 7) / 8;  // v is cut into m_tiles near-equal chunks of 8*m8 <= 128 rows
+    SIE_TRY(make_tensor_map_3d(&J.mapA, CvT, p.nao, p.v, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * p.v, 8, 8 * m8, 1));
+    SIE_TRY(make_tensor_map_3d(&J.mapB, H, p.nao, (uint64_t)p.o * pb, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * p.o * pb, 8,
+                               128, 1));
+    J.n_total = (long long)p.o * pb;
+    J.M = p.v;
+    J.m8 = m8;
+    J.m_tiles = (p.v + 8 * m8 - 1) / (8 * m8);
+    J.n_tiles = (int)((J.n_total + 127) / 128);
+    J.kblocks = (p.nao + 7) / 8;
+    J.out.base = Bmat + q0;
+    J.out.ld_m = (long long)p.o * p.naux_ld;
+    J.out.M = p.v;
+    J.out.inner = pb;
+    J.out.valid_inner = pb;
+    J.out.stride_outer = p.naux_ld;
+    J.out.n_lin_total = J.n_total;
+    return SIE_OK;
+}
+// assign tile ranges, upload the descriptors to `d_jobs` (stream-ordered) and launch ONE grouped GEMM over all of them
+int launch_jobs(std::vector<XJob>& jobs, bool packed, unsigned char* d_jobs, int num_sms, Prof& prof, int stage, cudaStream_t st) {
+    if (jobs.empty()) return SIE_OK;
+    long long t = 0;
+    for (XJob& J : jobs) {
+        J.tile_begin = (int)t;
+        t += (long long)J.m_tiles * J.n_tiles;
+        if (t > 0x7fffffff) return SIE_EINVAL;
+    }
+    SIE_CUDA(cudaMemcpyAsync(d_jobs, jobs.data(), jobs.size() * sizeof(XJob), cudaMemcpyHostToDevice, st));
+    ProfSpan ps(prof, stage, st);
+    return launch_xform_gemm(packed, reinterpret_cast<const XJob*>(d_jobs), (int)jobs.size(), (int)t, num_sms, st);
+}
+
+// Transform of aux rows [p0,p1) of ONE cluster into Bmat ([v][o][naux_ld]).  L points at row p0 (device, or host when
+// host_L: staged through the two-buffer ring on the copy stream, one A1 launch per staged chunk).  One A1 and one A2
+// launch per H sub-block otherwise.
 int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof, double* Bmat, const Scratch& sc, const double* dC_occ,
                    const double* dC_vir, const double* L, bool host_L, int p0, int p1, cudaStream_t st) {
     const int nao = p.nao, o = p.o, v = p.v;
@@ -361,86 +435,55 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
         }
         return SIE_OK;
     }
-    const int tm1 = gemm_tm_for(o), tm2 = gemm_tm_for(v);
-    const int kblocks = (nao + 7) / 8;
-    CUtensorMap mapCo, mapCv;
-    SIE_TRY(make_tensor_map_3d(&mapCo, sc.CoT, nao, o, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * o, 8, tm1, 1));
-    SIE_TRY(make_tensor_map_3d(&mapCv, sc.CvT, nao, v, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * v, 8, tm2, 1));
     if (host_L) {
         // the staging copies of this call must not start before earlier work on `st` that owns the workspace: ONE fork per
-        // call; after that only the per-buffer ready/consumed events order the ring, so the H2D copy of sub-block n+1 runs
-        // under the unpack/A1/A2 of sub-block n
+        // call; after that only the per-buffer ready/consumed events order the ring, so the H2D copy of chunk n+1 runs
+        // under the A1 of chunk n (and the A2 of the sub-block before)
         SIE_TRY(ensure_copy_pipeline(pipe_owner));
         SIE_CUDA(cudaEventRecord(pipe_owner.ev_fork, st));
         SIE_CUDA(cudaStreamWaitEvent(pipe_owner.copy_stream, pipe_owner.ev_fork, 0));
     }
+    unsigned char* arena = sc.jobs;
+    int used = 0;
+    std::vector<XJob> jobs(1);
     for (int q0 = p0; q0 < p1; q0 += p.pblk) {
         const int q1 = std::min(p1, q0 + p.pblk), pb = q1 - q0;
-        const double* Lq = L + (size_t)(q0 - p0) * p.npair;
-        if (host_L) {
-            // double-buffered H2D staging on a side stream, ordered against the unpack that consumes each buffer
-            sie_dfmp2_plan_s& po = pipe_owner;
-            const int buf = po.stage_turn & 1;
-            po.stage_turn++;
-            unsigned char* dst = sc.stage + (size_t)buf * sc.stage_buf_bytes;
-            SIE_CUDA(cudaStreamWaitEvent(po.copy_stream, po.ev_consumed[buf], 0));
-            SIE_CUDA(cudaMemcpyAsync(dst, Lq, (size_t)pb * p.npair * 8, cudaMemcpyHostToDevice, po.copy_stream));
-            SIE_CUDA(cudaEventRecord(po.ev_ready[buf], po.copy_stream));
-            SIE_CUDA(cudaStreamWaitEvent(st, po.ev_ready[buf], 0));
-            {
-                ProfSpan ps(prof, ST_UNPACK, st);
-                SIE_TRY(launch_unpack(reinterpret_cast<const double*>(dst), pb, nao, sc.Lfull, p.nao_ld, st));
+        const int step = host_L ? p.cblk : pb;
+        for (int c0 = q0; c0 < q1; c0 += step) {
+            const int c1 = std::min(q1, c0 + step), np = c1 - c0;
+            const double* Lq = L + (size_t)(c0 - p0) * p.npair;
+            int buf = 0;
+            if (host_L) {
+                sie_dfmp2_plan_s& po = pipe_owner;
+                buf = po.stage_turn++ & 1;
+                unsigned char* dst = sc.stage + (size_t)buf * sc.stage_buf_bytes;
+                SIE_CUDA(cudaStreamWaitEvent(po.copy_stream, po.ev_consumed[buf], 0));
+                SIE_CUDA(cudaMemcpyAsync(dst, Lq, (size_t)np * p.npair * 8, cudaMemcpyHostToDevice, po.copy_stream));
+                SIE_CUDA(cudaEventRecord(po.ev_ready[buf], po.copy_stream));
+                SIE_CUDA(cudaStreamWaitEvent(st, po.ev_ready[buf], 0));
+                Lq = reinterpret_cast<const double*>(dst);
             }
-            SIE_CUDA(cudaEventRecord(po.ev_consumed[buf], st));
-        } else {
-            ProfSpan ps(prof, ST_UNPACK, st);
-            SIE_TRY(launch_unpack(Lq, pb, nao, sc.Lfull, p.nao_ld, st));
+            if (used >= p.max_jobs) return SIE_EINVAL;  // cannot happen: max_jobs counts every chunk and sub-block
+            SIE_TRY(make_a1_job(jobs[0], p, sc.CoT, Lq, np, sc.H, c0 - q0, pb));
+            SIE_TRY(launch_jobs(jobs, true, arena + (size_t)used++ * sizeof(XJob), p.num_sms, prof, ST_T1, st));
+            if (host_L) SIE_CUDA(cudaEventRecord(pipe_owner.ev_consumed[buf], st));
         }
-        // A1: H[i][P][nu] = sum_mu CoT[i][mu] * Lfull[P][nu][mu].  The pb * nao rows (P, nu) of the unpacked block are
-        // contiguous, so the N dimension is tiled over the flat row index: no per-P padding of nao to 128
-        CUtensorMap mapL, mapH;
-        const uint64_t lrows = (uint64_t)pb * nao;
-        SIE_TRY(make_tensor_map_3d(&mapL, sc.Lfull, nao, lrows, 1, (uint64_t)p.nao_ld * 8, lrows * p.nao_ld * 8, 8, 128, 1));
-        GemmOut o1;
-        o1.base = sc.H;
-        o1.ld_m = (long long)pb * p.nao_ld;
-        o1.M = o;
-        o1.inner = nao;
-        o1.valid_inner = nao;
-        o1.stride_outer = p.nao_ld;
-        o1.n_lin_total = (long long)lrows;
-        const int n1_tiles = (int)((lrows + 127) / 128);
-        {
-            ProfSpan ps(prof, ST_T1, st);
-            SIE_TRY(launch_gemm_tn(tm1, mapCo, mapL, 1, n1_tiles, n1_tiles, 0, kblocks, o1, p.num_sms, st));
-        }
-        // A2: B[a][i][q0+P] = sum_nu CvT[a][nu] * H[(i,P)][nu]
-        SIE_TRY(make_tensor_map_3d(&mapH, sc.H, nao, (uint64_t)o * pb, 1, (uint64_t)p.nao_ld * 8,
-                                   (uint64_t)p.nao_ld * 8 * o * pb, 8, 128, 1));
-        GemmOut o2;
-        o2.base = Bmat + q0;
-        o2.ld_m = (long long)o * p.naux_ld;
-        o2.M = v;
-        o2.inner = pb;
-        o2.valid_inner = pb;
-        o2.stride_outer = p.naux_ld;
-        o2.n_lin_total = (long long)o * pb;
-        const int m_tiles = (v + tm2 - 1) / tm2, n_tiles = (int)(((long long)o * pb + 127) / 128);
-        {
-            ProfSpan ps(prof, ST_T2, st);
-            SIE_TRY(launch_gemm_tn(tm2, mapCv, mapH, m_tiles, n_tiles, n_tiles, 0, kblocks, o2, p.num_sms, st));
-        }
+        if (used >= p.max_jobs) return SIE_EINVAL;
+        SIE_TRY(make_a2_job(jobs[0], p, sc.CvT, sc.H, pb, Bmat, q0));
+        SIE_TRY(launch_jobs(jobs, false, arena + (size_t)used++ * sizeof(XJob), p.num_sms, prof, ST_T2, st));
     }
     return SIE_OK;
 }
 
+// transposed (K-major) copies of the coefficient matrices of one cluster
 int prepare_coeffs(sie_dfmp2_plan_s& p, Prof& prof, const Scratch& sc, const double* dC_occ, const double* dC_vir,
                    cudaStream_t st) {
     if (p.ref) return SIE_OK;
+    TJob tj[2] = {{dC_occ, sc.CoT, p.nao, p.o, p.nao_ld, 0}, {dC_vir, sc.CvT, p.nao, p.v, p.nao_ld, 0}};
+    unsigned char* d = sc.jobs + (size_t)p.max_jobs * sizeof(XJob);
+    SIE_CUDA(cudaMemcpyAsync(d, tj, sizeof tj, cudaMemcpyHostToDevice, st));
     ProfSpan ps(prof, ST_COEFF, st);
-    SIE_TRY(launch_transpose(dC_occ, p.nao, p.o, sc.CoT, p.nao_ld, st));
-    SIE_TRY(launch_transpose(dC_vir, p.nao, p.v, sc.CvT, p.nao_ld, st));
-    return SIE_OK;
+    return launch_transpose_jobs(reinterpret_cast<const TJob*>(d), 2, p.nao, std::max(p.o, p.v), st);
 }
 
 int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const double* de_occ, const double* de_vir, double* gpart,
@@ -461,44 +504,6 @@ int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const doubl
     d.tx_bytes = 2u * 8u * (uint32_t)p.t8 * 8u;
     return SIE_OK;
 }
-
-#ifndef SIE_BATCH_LANES
-#define SIE_BATCH_LANES 4
-#endif
-constexpr int BATCH_LANES = SIE_BATCH_LANES;
-
-// side streams of one batch call: forked from / joined into the caller's stream with events
-struct LaneStreams {
-    std::vector<cudaStream_t> streams;
-    std::vector<cudaEvent_t> done;
-    cudaEvent_t start = nullptr;
-    int fork(int n, cudaStream_t st) {
-        SIE_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
-        SIE_CUDA(cudaEventRecord(start, st));
-        for (int l = 0; l < n; ++l) {
-            cudaStream_t s;
-            cudaEvent_t e;
-            SIE_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
-            streams.push_back(s);
-            SIE_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-            done.push_back(e);
-            SIE_CUDA(cudaStreamWaitEvent(s, start, 0));
-        }
-        return SIE_OK;
-    }
-    int join(cudaStream_t st) {
-        for (size_t l = 0; l < streams.size(); ++l) {
-            SIE_CUDA(cudaEventRecord(done[l], streams[l]));
-            SIE_CUDA(cudaStreamWaitEvent(st, done[l], 0));
-        }
-        return SIE_OK;
-    }
-    ~LaneStreams() {  // destruction is deferred by the runtime until the enqueued work has completed
-        for (cudaEvent_t e : done) cudaEventDestroy(e);
-        if (start) cudaEventDestroy(start);
-        for (cudaStream_t s : streams) cudaStreamDestroy(s);
-    }
-};
 
 int check_gap_host(const double* e_occ, const double* e_vir, int o, int v) {
     double mo = e_occ[0], mv = e_vir[0];
@@ -526,7 +531,7 @@ int sie_dfmp2_plan(sie_dfmp2_plan_t* plan, int nao, int nocc, int nvir, int naux
     if (!p) return SIE_ENOMEM;
     int rc;
     try {
-        rc = plan_init(*p, nao, nocc, nvir, naux, aux_block, flags, true);
+        rc = plan_init(*p, nao, nocc, nvir, naux, aux_block, flags, CARVE_ALL);
     } catch (const std::bad_alloc&) {
         rc = SIE_ENOMEM;
     }
@@ -558,8 +563,8 @@ int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_
     Scratch sc{};
     sc.CoT = reinterpret_cast<double*>(ws + p.off_CoT);
     sc.CvT = reinterpret_cast<double*>(ws + p.off_CvT);
-    sc.Lfull = reinterpret_cast<double*>(ws + p.off_Lfull);
     sc.H = reinterpret_cast<double*>(ws + p.off_H);
+    sc.jobs = ws + p.off_jobs;
     sc.refH = reinterpret_cast<double*>(ws + p.off_refH);
     sc.stage = ws + p.off_stage;
     sc.stage_buf_bytes = p.stage_buf_bytes;
@@ -690,41 +695,50 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         return SIE_OK;
     }
     try {
-        // ---- per-cluster plans (B + partial-G regions) and shared scratch sized for the largest cluster
+        // ---- per-cluster plans.  Device pointers: every fused-path cluster owns B, partial-G slots, coefficient copies and
+        //      an H sub-block, so ONE grouped launch per transform stage serves all clusters.  Host pointers: the packed
+        //      integrals go through one staging ring, cluster by cluster, with shared scratch sized for the largest cluster.
         std::vector<sie_dfmp2_plan_s> plans(ncluster);
         Carver c;
         std::vector<size_t> off_cl(ncluster), off_io(ncluster);
-        size_t max_CoT = 0, max_CvT = 0, max_Lfull = 0, max_H = 0, max_refH = 0, max_refVj = 0, max_stage = 0, ntiles_total = 0;
+        size_t max_CoT = 0, max_CvT = 0, max_H = 0, max_refH = 0, max_refVj = 0, max_stage = 0, ntiles_total = 0, max_jobs1 = 0, group_jobs = 0;
+        int nfused = 0;
         for (int k = 0; k < ncluster; ++k) {
             const sie_dfmp2_cluster_t& cl = clusters[k];
             if (!query && (!cl.C_occ || !cl.C_vir || !cl.L_packed || !cl.e_occ || !cl.e_vir || !cl.E_out)) return SIE_EINVAL;
             sie_dfmp2_plan_s& p = plans[k];
-            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~(SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_OCC), false));
+            SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~(SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_OCC),
+                              host ? CARVE_NONE : CARVE_MEMBER));
             off_cl[k] = c.take(p.total);
             if (!p.ref) {
+                ++nfused;
                 max_CoT = std::max(max_CoT, (size_t)p.o * p.nao_ld * 8);
                 max_CvT = std::max(max_CvT, (size_t)p.v * p.nao_ld * 8);
-                max_Lfull = std::max(max_Lfull, (size_t)p.pblk * p.nao * p.nao_ld * 8);
                 max_H = std::max(max_H, (size_t)p.o * p.pblk * p.nao_ld * 8);
+                max_jobs1 = std::max(max_jobs1, (size_t)p.max_jobs);
+                group_jobs += 2 * (size_t)((p.naux + p.pblk - 1) / p.pblk);
                 ntiles_total += p.tiles.size();
             } else {
                 max_refH = std::max(max_refH, (size_t)p.pblk * p.o * p.nao * 8);
                 max_refVj = std::max(max_refVj, ref_vj_bytes(p.o, p.v));
             }
-            max_stage = std::max(max_stage, align_up((size_t)p.pblk * p.npair * 8, 256));
+            max_stage = std::max(max_stage, align_up((size_t)p.cblk * p.npair * 8, 256));
             if (host) {
                 size_t d = (size_t)p.nao * p.o + (size_t)p.nao * p.v + p.o + p.v + 2 * (size_t)p.o * p.o + 2;
                 off_io[k] = c.take(d * 8);
             }
         }
-        // transform lanes: the per-cluster transforms of a batch are many small launches (config 2: ~2900), so they are
-        // dealt to a few side streams with private scratch and run concurrently; the pair launch joins them
-        const int nlanes = (host || (flags & SIE_FLAG_VALIDATE)) ? 1 : std::min(BATCH_LANES, ncluster);
-        const size_t lane_bytes = align_up(max_CoT, 256) + align_up(max_CvT, 256) + align_up(max_Lfull, 256) + align_up(max_H, 256) +
-                                  align_up(max_refH, 256);
-        const size_t off_lanes = c.take(lane_bytes * nlanes);
+        size_t off_CoT = 0, off_CvT = 0, off_H = 0;
+        if (host) {
+            off_CoT = c.take(max_CoT);
+            off_CvT = c.take(max_CvT);
+            off_H = c.take(max_H);
+        }
+        const size_t off_refH = c.take(max_refH);
         const size_t off_refVj = c.take(max_refVj);
         const size_t off_stage = host ? c.take(2 * max_stage) : 0;
+        const size_t njobs_arena = host ? max_jobs1 : group_jobs;
+        const size_t off_jobs = c.take(njobs_arena * sizeof(XJob) + 2 * (size_t)std::max(1, ncluster) * sizeof(TJob));
         const size_t off_desc = c.take((size_t)std::max(1, ncluster) * sizeof(PairCluster));
         const size_t off_tiles = c.take(std::max<size_t>(1, ntiles_total) * sizeof(PairTile) + 256);
         const size_t off_rc = c.take((size_t)std::max(1, ncluster) * sizeof(ReduceCluster));
@@ -758,31 +772,17 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             }
         } guard{pipe};
 
-        std::vector<Scratch> lanes(nlanes);
-        for (int l = 0; l < nlanes; ++l) {
-            unsigned char* b = ws + off_lanes + (size_t)l * lane_bytes;
-            Scratch& sc = lanes[l];
-            sc.CoT = reinterpret_cast<double*>(b), b += align_up(max_CoT, 256);
-            sc.CvT = reinterpret_cast<double*>(b), b += align_up(max_CvT, 256);
-            sc.Lfull = reinterpret_cast<double*>(b), b += align_up(max_Lfull, 256);
-            sc.H = reinterpret_cast<double*>(b), b += align_up(max_H, 256);
-            sc.refH = reinterpret_cast<double*>(b);
-            sc.stage = ws + off_stage;
-            sc.stage_buf_bytes = max_stage;
-        }
-        LaneStreams ls;
-        if (nlanes > 1) SIE_TRY(ls.fork(nlanes, st));
-
         std::vector<PairCluster> descs(ncluster);
         std::vector<ReduceCluster> rcs(ncluster);
-        std::vector<const double*> de_occ(ncluster), de_vir(ncluster);
+        std::vector<const double*> de_occ(ncluster), de_vir(ncluster), dCo(ncluster), dCv(ncluster);
         std::vector<double*> dE(ncluster), dG(ncluster);
-        // ---- stage 1: per-cluster transforms (A1, A2)
+        // ---- stage 0: per-cluster pointers (host pointers: small operands uploaded; VALIDATE: gap check)
         for (int k = 0; k < ncluster; ++k) {
             const sie_dfmp2_cluster_t& cl = clusters[k];
             sie_dfmp2_plan_s& p = plans[k];
-            unsigned char* wk = ws + off_cl[k];
-            const double *dCo = cl.C_occ, *dCv = cl.C_vir, *dP = cl.P_frag;
+            const double* dP = cl.P_frag;
+            dCo[k] = cl.C_occ;
+            dCv[k] = cl.C_vir;
             de_occ[k] = cl.e_occ;
             de_vir[k] = cl.e_vir;
             dE[k] = cl.E_out;
@@ -796,12 +796,12 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                     d += n;
                     return cudaMemcpyAsync(dst, src, n * 8, cudaMemcpyHostToDevice, st) == cudaSuccess ? dst : nullptr;
                 };
-                dCo = up(cl.C_occ, (size_t)p.nao * p.o);
-                dCv = up(cl.C_vir, (size_t)p.nao * p.v);
+                dCo[k] = up(cl.C_occ, (size_t)p.nao * p.o);
+                dCv[k] = up(cl.C_vir, (size_t)p.nao * p.v);
                 de_occ[k] = up(cl.e_occ, p.o);
                 de_vir[k] = up(cl.e_vir, p.v);
                 if (cl.P_frag) dP = up(cl.P_frag, (size_t)p.o * p.o);
-                if (!dCo || !dCv || !de_occ[k] || !de_vir[k] || (cl.P_frag && !dP)) return set_cuda_error(cudaGetLastError());
+                if (!dCo[k] || !dCv[k] || !de_occ[k] || !de_vir[k] || (cl.P_frag && !dP)) return set_cuda_error(cudaGetLastError());
                 dE[k] = io + d;
                 d += 2;
                 dG[k] = cl.G_out ? io + d : nullptr;
@@ -812,11 +812,6 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                 SIE_CUDA(cudaStreamSynchronize(st));
                 SIE_TRY(check_gap_host(he.data(), he.data() + p.o, p.o, p.v));
             }
-            const int lane = k % nlanes;
-            cudaStream_t sk = nlanes > 1 ? ls.streams[lane] : st;
-            SIE_TRY(prepare_coeffs(p, prof, lanes[lane], dCo, dCv, sk));
-            SIE_TRY(transform_rows(p, pipe, prof, reinterpret_cast<double*>(wk + p.off_B), lanes[lane], dCo, dCv, cl.L_packed, host, 0,
-                                   p.naux, sk));
             rcs[k] = ReduceCluster{};
             rcs[k].P = dP;
             rcs[k].E_out = dE[k];
@@ -825,7 +820,79 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             rcs[k].mode = mode;
             if (mode) rcs[k].P = nullptr;
         }
-        if (nlanes > 1) SIE_TRY(ls.join(st));
+        // ---- stage 1: transforms (A1, A2)
+        unsigned char* arena = ws + off_jobs;
+        if (host) {
+            Scratch sc{};
+            sc.CoT = reinterpret_cast<double*>(ws + off_CoT);
+            sc.CvT = reinterpret_cast<double*>(ws + off_CvT);
+            sc.H = reinterpret_cast<double*>(ws + off_H);
+            sc.refH = reinterpret_cast<double*>(ws + off_refH);
+            sc.stage = ws + off_stage;
+            sc.stage_buf_bytes = max_stage;
+            for (int k = 0; k < ncluster; ++k) {
+                sie_dfmp2_plan_s& p = plans[k];
+                // this cluster's descriptors: max_jobs XJobs, then its two TJobs (prepare_coeffs expects them right behind)
+                sc.jobs = arena + (max_jobs1 - (size_t)p.max_jobs) * sizeof(XJob);
+                SIE_TRY(prepare_coeffs(p, prof, sc, dCo[k], dCv[k], st));
+                SIE_TRY(transform_rows(p, pipe, prof, reinterpret_cast<double*>(ws + off_cl[k] + p.off_B), sc, dCo[k], dCv[k],
+                                       clusters[k].L_packed, true, 0, p.naux, st));
+            }
+        } else {
+            // one transpose launch, then per round r (the r-th H sub-block of every cluster) ONE A1 and ONE A2 launch
+            std::vector<TJob> tj;
+            int max_rows = 1, max_cols = 1, rounds = 0;
+            for (int k = 0; k < ncluster; ++k) {
+                sie_dfmp2_plan_s& p = plans[k];
+                if (p.ref) continue;
+                unsigned char* wk = ws + off_cl[k];
+                tj.push_back(TJob{dCo[k], reinterpret_cast<double*>(wk + p.off_CoT), p.nao, p.o, p.nao_ld, 0});
+                tj.push_back(TJob{dCv[k], reinterpret_cast<double*>(wk + p.off_CvT), p.nao, p.v, p.nao_ld, 0});
+                max_rows = std::max(max_rows, p.nao);
+                max_cols = std::max(max_cols, std::max(p.o, p.v));
+                rounds = std::max(rounds, (p.naux + p.pblk - 1) / p.pblk);
+            }
+            if (!tj.empty()) {
+                unsigned char* d = arena + njobs_arena * sizeof(XJob);
+                SIE_CUDA(cudaMemcpyAsync(d, tj.data(), tj.size() * sizeof(TJob), cudaMemcpyHostToDevice, st));
+                ProfSpan ps(prof, ST_COEFF, st);
+                SIE_TRY(launch_transpose_jobs(reinterpret_cast<const TJob*>(d), (int)tj.size(), max_rows, max_cols, st));
+            }
+            size_t used = 0;
+            std::vector<XJob> j1, j2;
+            for (int r = 0; r < rounds; ++r) {
+                j1.clear();
+                j2.clear();
+                for (int k = 0; k < ncluster; ++k) {
+                    sie_dfmp2_plan_s& p = plans[k];
+                    if (p.ref) continue;
+                    const int q0 = r * p.pblk;
+                    if (q0 >= p.naux) continue;
+                    const int pb = std::min(p.pblk, p.naux - q0);
+                    unsigned char* wk = ws + off_cl[k];
+                    double* H = reinterpret_cast<double*>(wk + p.off_H);
+                    XJob J;
+                    SIE_TRY(make_a1_job(J, p, reinterpret_cast<const double*>(wk + p.off_CoT), clusters[k].L_packed + (size_t)q0 * p.npair, pb,
+                                        H, 0, pb));
+                    j1.push_back(J);
+                    SIE_TRY(make_a2_job(J, p, reinterpret_cast<const double*>(wk + p.off_CvT), H, pb, reinterpret_cast<double*>(wk + p.off_B), q0));
+                    j2.push_back(J);
+                }
+                if (used + j1.size() + j2.size() > njobs_arena) return SIE_EINVAL;  // cannot happen: counted above
+                SIE_TRY(launch_jobs(j1, true, arena + used * sizeof(XJob), plans[0].num_sms, prof, ST_T1, st));
+                used += j1.size();
+                SIE_TRY(launch_jobs(j2, false, arena + used * sizeof(XJob), plans[0].num_sms, prof, ST_T2, st));
+                used += j2.size();
+            }
+            for (int k = 0; k < ncluster; ++k) {  // reference-path clusters: simple kernels, one cluster at a time
+                sie_dfmp2_plan_s& p = plans[k];
+                if (!p.ref) continue;
+                Scratch sc{};
+                sc.refH = reinterpret_cast<double*>(ws + off_refH);
+                SIE_TRY(transform_rows(p, pipe, prof, reinterpret_cast<double*>(ws + off_cl[k] + p.off_B), sc, dCo[k], dCv[k],
+                                       clusters[k].L_packed, false, 0, p.naux, st));
+            }
+        }
         // ---- stage 2: one persistent pair launch over all (cluster, tile) items, most expensive tiles first
         std::vector<int> order;
         for (int k = 0; k < ncluster; ++k)

@@ -9,11 +9,6 @@
 namespace sie {
 
 // ---- transform.cu ------------------------------------------------------------------------------
-// out[c][r] = in[r][c] for r < rows, c < cols; out has leading dimension ld_out (>= rows).
-int launch_transpose(const double* in, int rows, int cols, double* out, int ld_out, cudaStream_t st);
-// packed lower triangles [np][nao(nao+1)/2] -> full symmetric [np][nao][ld] (ld >= nao)
-int launch_unpack(const double* Lp, int np, int nao, double* Lfull, int ld, cudaStream_t st);
-
 struct GemmOut {
     double* base;          // output base pointer
     long long ld_m;        // offset per row m
@@ -23,13 +18,27 @@ struct GemmOut {
     long long stride_outer;  // offset = outer * stride_outer + rem
     long long n_lin_total;   // column valid iff n_lin < n_lin_total
 };
-// C = A * B^T with K-major operands described by 3-D tensor maps (box {8, rows, 1}); tile nb of the B operand
-// sits at coordinates (k, (nb % nb_inner) * TN, nb / nb_inner) and its first column has
-// n_lin = (nb / nb_inner) * inner_pad + (nb % nb_inner) * TN.
-// tm_sel picks the M-tile height: 16, 32, 64 or 128 (TN is always 128).
-int launch_gemm_tn(int tm_sel, const CUtensorMap& mapA, const CUtensorMap& mapB, int m_tiles, int n_tiles, int nb_inner,
-                   long long inner_pad, int kblocks, const GemmOut& out, int num_sms, cudaStream_t st);
-int gemm_tm_for(int m);  // smallest supported M-tile height covering min(m,128)
+// One GEMM of a grouped launch: C[m][n] = sum_k A[m][k] * Bop[n][k], K-major operands (transform.cu)
+struct alignas(128) XJob {
+    CUtensorMap mapA;       // K-major A operand [M][K], box {8, 8*m8, 1}
+    CUtensorMap mapB;       // TMA mode: K-major Bop [N][K], box {8, 128, 1}
+    const double* Lp;       // packed mode: [np][npair]
+    long long npair;
+    long long n_total;      // valid flat columns n
+    int nao;                // packed mode: n = P * nao + nu
+    int M, m8, m_tiles, n_tiles, kblocks;
+    int tile_begin;         // global index of this job's first tile (tiles of a job: m fastest)
+    GemmOut out;
+};
+
+int launch_xform_gemm(bool packed, const XJob* d_jobs, int njobs, int total_tiles, int num_sms, cudaStream_t st);
+// one coefficient transpose of a grouped launch: out[c][r] = in[r][c] for r < rows, c < cols, leading dimension ld_out
+struct TJob {
+    const double* in;
+    double* out;
+    int rows, cols, ld_out, pad;
+};
+int launch_transpose_jobs(const TJob* d_jobs, int njobs, int max_rows, int max_cols, cudaStream_t st);
 
 // ---- pair.cu -----------------------------------------------------------------------------------
 struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (global memory)
