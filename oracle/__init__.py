@@ -32,6 +32,8 @@ def lib() -> ctypes.CDLL:
         L.sie_oracle_pair_G.restype = ctypes.c_int
         L.sie_oracle_rdm_occ.argtypes = [ctypes.c_int] * 3 + [dp, dp, dp, dp]
         L.sie_oracle_rdm_occ.restype = ctypes.c_int
+        L.sie_oracle_rdm_vir.argtypes = [ctypes.c_int] * 3 + [dp, dp, dp, dp]
+        L.sie_oracle_rdm_vir.restype = ctypes.c_int
         L.sie_oracle_trace.argtypes = [ctypes.c_int, dp, dp]
         L.sie_oracle_trace.restype = ctypes.c_double
         _lib = L
@@ -111,6 +113,18 @@ def rdm_occ(B, e_occ, e_vir) -> np.ndarray:
     rc = lib().sie_oracle_rdm_occ(nocc, nvir, naux, _p(B), _p(e_occ), _p(e_vir), _p(g))
     if rc != 0:
         raise MemoryError("sie_oracle_rdm_occ")
+    return g
+
+
+def rdm_vir(B, e_occ, e_vir) -> np.ndarray:
+    """Virtual block of the MP2 1-RDM, gamma_ab of PAPER.md Eq. S17 (L355): [nvir][nvir]."""
+    B, e_occ, e_vir = _c(B), _c(e_occ), _c(e_vir)
+    nocc, nvir, naux = B.shape
+    assert e_occ.shape == (nocc,) and e_vir.shape == (nvir,)
+    g = np.empty((nvir, nvir))
+    rc = lib().sie_oracle_rdm_vir(nocc, nvir, naux, _p(B), _p(e_occ), _p(e_vir), _p(g))
+    if rc != 0:
+        raise MemoryError("sie_oracle_rdm_vir")
     return g
 
 

@@ -25,8 +25,8 @@
  * of O4 uses 8 explicit partial sums (still a plain loop); the (a,b), j and trace accumulations are
  * carried in long double so the oracle's own rounding sits far below the GPU's.
  *
- * NEXT-1 addition at the end of this file: O8 gamma_ij, occupied block of the MP2 1-RDM (Eq. S18), pinned in
- * tests/test_oracle_rdm_pins.py.
+ * NEXT-1 additions at the end of this file: O8 gamma_ij and O9 gamma_ab, occupied and virtual blocks of the MP2 1-RDM
+ * (Eq. S18, S17), pinned in tests/test_oracle_rdm_pins.py.
  *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): hand-worked 2x1 and 1x1 cases
  * (tests/golden/handworked.txt), closed form o=v=1, P=I == textbook closed-shell MP2 from brute-force
@@ -232,6 +232,48 @@ int sie_oracle_rdm_occ(int nocc, int nvir, int naux, const double* B, const doub
         for (int j = 0; j < nocc; ++j)
             gamma[(size_t)i * nocc + j] = (double)((i == j ? 2.0L : 0.0L) - 2.0L * Gl[(size_t)i * nocc + j]);
     free(Tk);
+    free(Gl);
+    return 0;
+}
+
+/*
+ * NEXT-1: virtual block of the MP2 one-particle reduced density matrix, PAPER.md Eq. S17 (L355):
+ *     gamma_ab = 2 sum_ij sum_c t_ij^ac ( 2 t_ij^bc - t_ij^cb ),        t_ij^ac = (ia|jc) / (e_i + e_j - e_a - e_c)
+ * (Eq. S15-S16; the sign of t cancels in the quadratic form).  The sub-space of Eq. S13-S14 (L338-L343) is
+ * whatever orbital sets the caller put into B: impurity-occupied x environment-virtual for the virtual BNOs.
+ *   B [nocc][nvir][naux], e_occ[nocc], e_vir[nvir]; gamma [nvir][nvir] row-major, OVERWRITTEN.
+ * Loops in the paper's order: for each pair (i, j) the amplitude block t_ij^{ac} (nvir x nvir), then every (a, b) with the
+ * sum over c; long-double accumulation.  Returns 0, or 1 on allocation failure.
+ * Pins: tests/test_oracle_rdm_pins.py (closed form o=v=1, hand-worked case, brute force from explicit four-index amplitudes,
+ * Tr gamma_occ + Tr gamma_vir = 2 nocc, gamma_aa = dE/de_a against the pinned energy, symmetry, positive semi-definiteness).
+ */
+int sie_oracle_rdm_vir(int nocc, int nvir, int naux, const double* B, const double* e_occ, const double* e_vir,
+                       double* gamma) {
+    const size_t vv = (size_t)nvir * nvir;
+    double* T = (double*)malloc(sizeof(double) * vv);                      /* t_ij^ac for one (i, j) */
+    long double* Gl = (long double*)calloc(vv, sizeof(long double));
+    if (!T || !Gl) { free(T); free(Gl); return 1; }
+    for (int i = 0; i < nocc; ++i)
+        for (int j = 0; j < nocc; ++j) {
+#pragma omp parallel for schedule(static)
+            for (int a = 0; a < nvir; ++a) {
+                const double* bia = B + ((size_t)i * nvir + a) * naux;
+                for (int c = 0; c < nvir; ++c)
+                    T[(size_t)a * nvir + c] =
+                        dot8(bia, B + ((size_t)j * nvir + c) * naux, naux) / (e_occ[i] + e_occ[j] - e_vir[a] - e_vir[c]);
+            }
+#pragma omp parallel for collapse(2) schedule(static)
+            for (int a = 0; a < nvir; ++a)
+                for (int b = 0; b < nvir; ++b) {
+                    long double s = 0.0L;
+                    for (int c = 0; c < nvir; ++c)
+                        s += (long double)T[(size_t)a * nvir + c] *
+                             (2.0L * (long double)T[(size_t)b * nvir + c] - (long double)T[(size_t)c * nvir + b]);
+                    Gl[(size_t)a * nvir + b] += s;
+                }
+        }
+    for (size_t k = 0; k < vv; ++k) gamma[k] = (double)(2.0L * Gl[k]);
+    free(T);
     free(Gl);
     return 0;
 }
