@@ -56,8 +56,9 @@ enum {
     SIE_FLAG_REFERENCE = 2u, /* use the simple FP64-FMA reference kernels (any nocc; slow; cross-check path) */
     SIE_FLAG_HOST_IO = 4u,   /* data pointers are HOST pointers; the library stages H2D/D2H copies */
     SIE_FLAG_PROFILE = 8u,   /* bracket every launch group with CUDA events; read with *_timing (below) */
-    SIE_FLAG_RDM_OCC = 16u   /* sie_dfmp2_batch only: compute the occupied 1-RDM block of every cluster instead of the
+    SIE_FLAG_RDM_OCC = 16u,  /* sie_dfmp2_batch only: compute the occupied 1-RDM block of every cluster instead of the
                                 energy (3b): G_out receives gamma, E_out receives Tr gamma, P_frag is ignored */
+    SIE_FLAG_RDM_VIR = 32u   /* sie_dfmp2_plan only: reserve the workspace sie_dfmp2_rdm_vir (3c) needs (three amplitude slabs) */
 };
 
 /*
@@ -65,7 +66,13 @@ enum {
  *    sub-block (the rows of the half-transformed intermediate H that exist at once; at most 2 GB), and reports the device workspace (bytes, 256-byte aligned base required) the caller must
  *    pass to transform/energy.  The workspace holds B[a][i][P] between transform and energy.
  *      nao >= nocc + nvir, nocc >= 1, nvir >= 1, naux >= 1; aux_block = rows of (P|mu nu) processed per
- *      internal step (0 = auto).  nocc > 128 silently selects the reference kernels.
+ *      internal step (0 = auto).
+ *    Three routes exist for the pair stage, reported by sie_dfmp2_plan_info()[7]:
+ *      0 fused      nocc <= 128: one persistent kernel, V and t never leave the chip (the tuned path)
+ *      2 general    nocc > 128 (e.g. the environment-occupied sub-space of PAPER.md Eq. S13): per occupied block a
+ *                   slab GEMM, an amplitude pass and a split-K Gram GEMM, all on the FP64 tensor cores; the amplitude slab of
+ *                   one occupied block (nvir^2 * nocc * block doubles, <= 4 GB or SIE_EINVAL) is the largest intermediate
+ *      1 reference  SIE_FLAG_REFERENCE: simple FP64-FMA kernels, a cross-check only
  */
 int sie_dfmp2_plan(sie_dfmp2_plan_t* plan, int nao, int nocc, int nvir, int naux, int aux_block,
                    unsigned flags, size_t* workspace_bytes);
@@ -101,6 +108,18 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
  *    after sie_dfmp2_energy on the same transformed workspace, any number of times.
  */
 int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir,
+                      double* gamma_out, double* trace_out, void* cuda_stream);
+
+/*
+ * 3c. sie_dfmp2_rdm_vir — NEXT-1: virtual block of the MP2 one-particle reduced density matrix, PAPER.md Eq. S17 (L355):
+ *        gamma_ab = 2 sum_ij sum_c t_ij^ac (2 t_ij^bc - t_ij^cb),   t_ij^ac = (ia|jc) / (e_i + e_j - e_a - e_c)
+ *    (the matrix whose eigenvectors rank the virtual bath natural orbitals; with the impurity-occupied x environment-virtual
+ *    orbital sets of Eq. S14, as C_occ / C_vir).  Runs on the general route at every size and needs a plan created
+ *    with SIE_FLAG_RDM_VIR (SIE_ESTATE otherwise; SIE_EUNSUPPORTED with SIE_FLAG_REFERENCE).
+ *      gamma_out [nvir][nvir] row-major (symmetric), REQUIRED;  trace_out: 1 double or NULL, receives Tr gamma_vir
+ *      (= 2 nocc - Tr gamma_occ).  Pointers, call order and errors as sie_dfmp2_rdm_occ.
+ */
+int sie_dfmp2_rdm_vir(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir,
                       double* gamma_out, double* trace_out, void* cuda_stream);
 
 /*
@@ -155,7 +174,7 @@ unsigned long long sie_dfmp2_launch_count(void);
  * Introspection for benchmarks/tests: fills info[0..n) with plan facts, returns how many exist.
  *   0, 1: pair-tile rows / cols in rows of B, ceil8(ta*nocc) <= 128   2: virtual blocks per tile side (ta)
  *   3: ceil8(nocc), the leading dimension of a partial-G slot   4: number of pair tiles   5: persistent CTAs   6: internal aux sub-block
- *   7: 1 if the reference kernels are selected
+ *   7: pair-stage route: 0 fused, 1 reference kernels, 2 general (nocc > 128)
  */
 int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n);
 

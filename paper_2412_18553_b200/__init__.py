@@ -7,6 +7,7 @@ from .binding import (  # noqa: F401
     SIE_FLAG_HOST_IO,
     SIE_FLAG_PROFILE,
     SIE_FLAG_RDM_OCC,
+    SIE_FLAG_RDM_VIR,
     SIE_FLAG_REFERENCE,
     SIE_FLAG_VALIDATE,
     ClusterSolver,
@@ -18,6 +19,7 @@ from .binding import (  # noqa: F401
     sie_dfmp2_destroy,
     sie_dfmp2_energy,
     sie_dfmp2_rdm_occ,
+    sie_dfmp2_rdm_vir,
     sie_dfmp2_plan,
     sie_dfmp2_plan_info,
     sie_dfmp2_plan_reset,

@@ -13,7 +13,7 @@ from typing import List, Optional, Sequence, Tuple
 import torch
 
 SIE_OK, SIE_EINVAL, SIE_ENOMEM, SIE_ECUDA, SIE_ESTATE, SIE_EGAP, SIE_EUNSUPPORTED = range(7)
-SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO, SIE_FLAG_PROFILE, SIE_FLAG_RDM_OCC = 1, 2, 4, 8, 16
+SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO, SIE_FLAG_PROFILE, SIE_FLAG_RDM_OCC, SIE_FLAG_RDM_VIR = 1, 2, 4, 8, 16, 32
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsie_dfmp2.so")
@@ -23,6 +23,7 @@ EXPORTS = (
     "sie_dfmp2_transform",
     "sie_dfmp2_energy",
     "sie_dfmp2_rdm_occ",
+    "sie_dfmp2_rdm_vir",
     "sie_dfmp2_batch",
     "sie_dfmp2_plan_reset",
     "sie_dfmp2_destroy",
@@ -84,6 +85,8 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_energy.restype = ci
         L.sie_dfmp2_rdm_occ.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.sie_dfmp2_rdm_occ.restype = ci
+        L.sie_dfmp2_rdm_vir.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.sie_dfmp2_rdm_vir.restype = ci
         L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
         L.sie_dfmp2_batch.restype = ci
         L.sie_dfmp2_plan_reset.argtypes = [vp]
@@ -163,6 +166,16 @@ def sie_dfmp2_rdm_occ(plan: int, workspace: torch.Tensor, e_occ, e_vir, gamma_ou
     )
 
 
+def sie_dfmp2_rdm_vir(plan: int, workspace: torch.Tensor, e_occ, e_vir, gamma_out, trace_out=None, *, host=False, stream=None) -> None:
+    """Virtual block of the MP2 1-RDM (PAPER.md Eq. S17); the plan needs SIE_FLAG_RDM_VIR; marshalling only."""
+    _check(
+        _lib().sie_dfmp2_rdm_vir(
+            plan, workspace.data_ptr(), _ptr(e_occ, host, "e_occ"), _ptr(e_vir, host, "e_vir"), _ptr(gamma_out, host, "gamma_out"),
+            _ptr(trace_out, host, "trace_out"), _stream_ptr(stream)),
+        "sie_dfmp2_rdm_vir",
+    )
+
+
 def sie_dfmp2_energy(plan: int, workspace: torch.Tensor, e_occ, e_vir, P_frag, E_out, G_out, *, host=False, stream=None) -> None:
     _check(
         _lib().sie_dfmp2_energy(
@@ -184,8 +197,10 @@ def sie_dfmp2_destroy(plan: Optional[int]) -> None:
 def sie_dfmp2_plan_info(plan: int) -> dict:
     buf = (ctypes.c_longlong * 8)()
     n = _lib().sie_dfmp2_plan_info(plan, buf, 8)
-    keys = ("TM", "TN", "ta", "o8", "ntiles", "ncta", "aux_subblock", "reference")
-    return {k: int(buf[i]) for i, k in enumerate(keys[:n])}
+    keys = ("TM", "TN", "ta", "o8", "ntiles", "ncta", "aux_subblock", "route")
+    d = {k: int(buf[i]) for i, k in enumerate(keys[:n])}
+    d["reference"], d["general"] = int(d.get("route") == 1), int(d.get("route") == 2)  # pair-stage route: 0 fused, 1 reference, 2 general
+    return d
 
 
 STAGES = ("coeff_transpose", "unpack", "A1_gemm", "A2_gemm", "pair", "reduce", "reference")
@@ -293,6 +308,16 @@ class ClusterSolver:
         if self.host:
             g, tr = g.pin_memory(), tr.pin_memory()
         sie_dfmp2_rdm_occ(self.plan, self.workspace, e_occ, e_vir, g, tr, host=self.host, stream=stream)
+        return g, tr
+
+    def rdm_vir(self, e_occ, e_vir, stream=None):
+        """-> (gamma_vir [nvir][nvir], Tr gamma_vir); the solver must have been created with SIE_FLAG_RDM_VIR"""
+        dev = "cpu" if self.host else self.device
+        g = torch.empty(self.nvir, self.nvir, dtype=torch.float64, device=dev)
+        tr = torch.empty(1, dtype=torch.float64, device=dev)
+        if self.host:
+            g, tr = g.pin_memory(), tr.pin_memory()
+        sie_dfmp2_rdm_vir(self.plan, self.workspace, e_occ, e_vir, g, tr, host=self.host, stream=stream)
         return g, tr
 
     def timing(self) -> dict:

@@ -196,7 +196,9 @@ struct sie_dfmp2_plan_s {
     Prof prof;
     int nao = 0, o = 0, v = 0, naux = 0;
     unsigned flags = 0;
-    bool ref = false;
+    bool ref = false, general = false, fused = true, has_gen = false;
+    GeneralGeom gen{};
+    size_t off_gen = 0, off_gslots = 0;
     int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, t8 = 8, nblk = 0, pblk = 0, cblk = 0, max_jobs = 0, ncta = 0, kp = 1, num_sms = 148;
     size_t npair = 0;
     std::vector<PairTile> tiles;  // cluster field = 0; rewritten when used inside a batch
@@ -248,7 +250,7 @@ enum { CARVE_NONE = 0, CARVE_MEMBER = 1, CARVE_ALL = 2 };  // what plan_init lay
 int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags, int carve) {
     if (nao < 1 || nocc < 1 || nvir < 1 || naux < 1 || aux_block < 0) return SIE_EINVAL;
     if ((long long)nocc + nvir > nao) return SIE_EINVAL;
-    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE)) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_VIR)) return SIE_EINVAL;
     p.nao = nao;
     p.o = nocc;
     p.v = nvir;
@@ -257,7 +259,9 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
     p.npair = (size_t)nao * (nao + 1) / 2;
     p.num_sms = query_num_sms();
     const PairGeom geo = pair_geom();
-    p.ref = (flags & SIE_FLAG_REFERENCE) || nocc > geo.TM;
+    p.ref = (flags & SIE_FLAG_REFERENCE) != 0;
+    p.general = !p.ref && nocc > geo.TM;  // an o x o block no longer fits one CTA tile: slab/Gram route (general.cu)
+    p.fused = !p.ref && !p.general;
     p.nao_ld = (int)align_up((size_t)nao, 8);
     p.naux_ld = (int)align_up((size_t)naux, 8);
     p.o8 = (int)align_up((size_t)nocc, 8);
@@ -278,7 +282,7 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
         long long cb = std::max<long long>(8, (long long)(((size_t)512 << 20) / (p.npair * 8)) / 8 * 8);
         p.cblk = (int)std::min<long long>(cb, p.pblk);
     }
-    if (!p.ref) {
+    if (p.fused) {
         // pair tiling: ta whole virtual blocks (ta*o <= 128 rows of B, o itself is never padded) per tile edge
         p.ta = std::max(1, geo.TM / nocc);
         p.t8 = (int)align_up((size_t)p.ta * nocc, 8);
@@ -294,10 +298,17 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
     // workspace
     Carver c;
     p.off_B = c.take((size_t)nvir * nocc * p.naux_ld * 8);
-    if (!p.ref)
+    if (p.fused)
         p.off_gpart = c.take(p.gpart_bytes);
-    else
+    else if (p.ref)
         p.off_refG = c.take((size_t)nocc * nocc * 8);
+    if (!p.ref && (p.general || (flags & SIE_FLAG_RDM_VIR))) {
+        p.gen = general_geom(nocc, nvir, p.num_sms);
+        if (!p.gen.ok) return SIE_EINVAL;  // one amplitude slab (nvir^2 * nocc doubles) would exceed 4 GB
+        p.has_gen = true;
+        p.off_gslots = c.take(p.gen.slots_bytes);
+        if (carve == CARVE_ALL) p.off_gen = c.take(general_scratch_bytes(p.gen, nocc));
+    }
     // job descriptors of one transform call: one A1 job per staged chunk (HOST_IO) or per sub-block, one A2 job per sub-block
     p.max_jobs = (naux + p.pblk - 1) / p.pblk + (naux + p.cblk - 1) / p.cblk + 8;
     if (carve == CARVE_MEMBER && !p.ref) {  // member of a device-pointer batch: private coefficient copies and H
@@ -328,7 +339,7 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
             p.io_ev = d, d += nvir;
             p.io_P = d, d += (size_t)nocc * nocc;
             p.io_E = d, d += 2;
-            p.io_G = d, d += (size_t)nocc * nocc;
+            p.io_G = d, d += std::max((size_t)nocc * nocc, (flags & SIE_FLAG_RDM_VIR) ? (size_t)nvir * nvir : (size_t)0);
             p.io_doubles = d;
             p.off_io = c.take(d * 8);
         }
@@ -359,7 +370,8 @@ struct Scratch {  // transform scratch of one cluster (device pointers)
 // A1 on `np` packed rows starting at Lq: H[i][P][nu] for P in [h0, h0+np) of an H sub-block that holds pbH rows
 int make_a1_job(XJob& J, const sie_dfmp2_plan_s& p, const double* CoT, const double* Lq, int np, double* H, int h0, int pbH) {
     std::memset(&J, 0, sizeof J);
-    const int m8 = p.o8 / 8;
+    const int m_tiles = (p.o + 127) / 128;
+    const int m8 = ((p.o + m_tiles - 1) / m_tiles + 7) / 8;  // o is cut into m_tiles near-equal chunks of 8*m8 <= 128 rows
     SIE_TRY(make_tensor_map_3d(&J.mapA, CoT, p.nao, p.o, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * p.o, 8, 8 * m8, 1));
     J.Lp = Lq;
     J.npair = (long long)p.npair;
@@ -367,7 +379,7 @@ int make_a1_job(XJob& J, const sie_dfmp2_plan_s& p, const double* CoT, const dou
     J.n_total = (long long)np * p.nao;
     J.M = p.o;
     J.m8 = m8;
-    J.m_tiles = 1;
+    J.m_tiles = (p.o + 8 * m8 - 1) / (8 * m8);
     J.n_tiles = (int)((J.n_total + 127) / 128);
     J.kblocks = (p.nao + 7) / 8;
     J.out.base = H + (size_t)h0 * p.nao_ld;
@@ -388,6 +400,7 @@ int make_a2_job(XJob& J, const sie_dfmp2_plan_s& p, const double* CvT, const dou
     SIE_TRY(make_tensor_map_3d(&J.mapB, H, p.nao, (uint64_t)p.o * pb, 1, (uint64_t)p.nao_ld * 8, (uint64_t)p.nao_ld * 8 * p.o * pb, 8,
                                128, 1));
     J.n_total = (long long)p.o * pb;
+    J.b_c1_mul = 128;
     J.M = p.v;
     J.m8 = m8;
     J.m_tiles = (p.v + 8 * m8 - 1) / (8 * m8);
@@ -639,6 +652,19 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
         rc.gpart = G;
         rc.o8 = o;
         rc.nslots = 1;
+    } else if (p.general || mode == 2) {
+        // any-size route (general.cu): nocc > 128, and the virtual 1-RDM block at every size
+        if (!p.has_gen) return SIE_ESTATE;  // gamma_vir needs a plan created with SIE_FLAG_RDM_VIR
+        double* slots = reinterpret_cast<double*>(ws + p.off_gslots);
+        int nslots = 0;
+        {
+            ProfSpan ps(p.prof, ST_PAIR, st);
+            SIE_TRY(general_pair(p.gen, Bmat, o, v, p.naux, p.naux_ld, de_occ, de_vir, mode, ws + p.off_gen, slots, &nslots, p.num_sms, st));
+        }
+        rc.gpart = slots;
+        rc.o = mode == 2 ? v : o;
+        rc.o8 = rc.o;
+        rc.nslots = nslots;
     } else {
         double* gpart = reinterpret_cast<double*>(ws + p.off_gpart);
         PairCluster pc;
@@ -665,7 +691,7 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
     }
     if (host) {
         if (E_out) SIE_CUDA(cudaMemcpyAsync(E_out, dE, 8, cudaMemcpyDeviceToHost, st));
-        if (G_out) SIE_CUDA(cudaMemcpyAsync(G_out, dG, (size_t)o * o * 8, cudaMemcpyDeviceToHost, st));
+        if (G_out) SIE_CUDA(cudaMemcpyAsync(G_out, dG, (size_t)rc.o * rc.o * 8, cudaMemcpyDeviceToHost, st));
         SIE_CUDA(cudaStreamSynchronize(st));
     }
     return SIE_OK;
@@ -680,6 +706,13 @@ int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_oc
                       double* trace_out, void* cuda_stream) {
     if (!gamma_out) return SIE_EINVAL;
     return energy_impl(plan, workspace, e_occ, e_vir, nullptr, trace_out, gamma_out, cuda_stream, 1);
+}
+
+int sie_dfmp2_rdm_vir(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, double* gamma_out,
+                      double* trace_out, void* cuda_stream) {
+    if (!gamma_out) return SIE_EINVAL;
+    if (plan && plan->ref) return SIE_EUNSUPPORTED;  // the reference kernels have no virtual-block mode
+    return energy_impl(plan, workspace, e_occ, e_vir, nullptr, trace_out, gamma_out, cuda_stream, 2);
 }
 
 int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* workspace, size_t workspace_bytes, size_t* needed,
@@ -701,7 +734,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         std::vector<sie_dfmp2_plan_s> plans(ncluster);
         Carver c;
         std::vector<size_t> off_cl(ncluster), off_io(ncluster);
-        size_t max_CoT = 0, max_CvT = 0, max_H = 0, max_refH = 0, max_refVj = 0, max_stage = 0, ntiles_total = 0, max_jobs1 = 0, group_jobs = 0;
+        size_t max_CoT = 0, max_CvT = 0, max_H = 0, max_refH = 0, max_refVj = 0, max_stage = 0, ntiles_total = 0, max_jobs1 = 0, group_jobs = 0, max_gen = 0;
         int nfused = 0;
         for (int k = 0; k < ncluster; ++k) {
             const sie_dfmp2_cluster_t& cl = clusters[k];
@@ -722,6 +755,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                 max_refH = std::max(max_refH, (size_t)p.pblk * p.o * p.nao * 8);
                 max_refVj = std::max(max_refVj, ref_vj_bytes(p.o, p.v));
             }
+            if (p.has_gen) max_gen = std::max(max_gen, general_scratch_bytes(p.gen, p.o));
             max_stage = std::max(max_stage, align_up((size_t)p.cblk * p.npair * 8, 256));
             if (host) {
                 size_t d = (size_t)p.nao * p.o + (size_t)p.nao * p.v + p.o + p.v + 2 * (size_t)p.o * p.o + 2;
@@ -736,6 +770,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         }
         const size_t off_refH = c.take(max_refH);
         const size_t off_refVj = c.take(max_refVj);
+        const size_t off_gen = c.take(max_gen);
         const size_t off_stage = host ? c.take(2 * max_stage) : 0;
         const size_t njobs_arena = host ? max_jobs1 : group_jobs;
         const size_t off_jobs = c.take(njobs_arena * sizeof(XJob) + 2 * (size_t)std::max(1, ncluster) * sizeof(TJob));
@@ -896,7 +931,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         // ---- stage 2: one persistent pair launch over all (cluster, tile) items, most expensive tiles first
         std::vector<int> order;
         for (int k = 0; k < ncluster; ++k)
-            if (!plans[k].ref) order.push_back(k);
+            if (plans[k].fused) order.push_back(k);
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return plans[a].tile_cost > plans[b].tile_cost; });
         const int ncta = (int)std::min<size_t>((size_t)plans[0].num_sms, std::max<size_t>(1, ntiles_total));
         std::vector<PairTile> tiles;
@@ -925,7 +960,23 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
                                 (int)tiles.size(), ncta, tmax, mode, st));
         }
-        // reference-path clusters (nocc > 128 or SIE_FLAG_REFERENCE): per-j kernels, one cluster at a time
+        // clusters with nocc > 128: the any-size slab/Gram route, one cluster at a time on shared scratch
+        for (int k = 0; k < ncluster; ++k) {
+            sie_dfmp2_plan_s& p = plans[k];
+            if (!p.general) continue;
+            unsigned char* wk = ws + off_cl[k];
+            double* slots = reinterpret_cast<double*>(wk + p.off_gslots);
+            int nslots = 0;
+            {
+                ProfSpan ps(prof, ST_PAIR, st);
+                SIE_TRY(general_pair(p.gen, reinterpret_cast<const double*>(wk + p.off_B), p.o, p.v, p.naux, p.naux_ld, de_occ[k], de_vir[k],
+                                     mode, ws + off_gen, slots, &nslots, p.num_sms, st));
+            }
+            rcs[k].gpart = slots;
+            rcs[k].o8 = p.o;
+            rcs[k].nslots = nslots;
+        }
+        // reference-path clusters (SIE_FLAG_REFERENCE): per-j kernels, one cluster at a time
         for (int k = 0; k < ncluster; ++k) {
             sie_dfmp2_plan_s& p = plans[k];
             if (!p.ref) continue;
@@ -1035,7 +1086,8 @@ int sie_dfmp2_probe_fp64(int kind, int iters, int ctas_per_sm, void* scratch, do
 int sie_dfmp2_plan_info(sie_dfmp2_plan_t plan, long long* info, int n) {
     if (!plan) return 0;
     const PairGeom geo = pair_geom();
-    const long long vals[8] = {plan->t8, plan->t8, plan->ta, plan->o8, (long long)plan->tiles.size(), plan->ncta, plan->pblk, plan->ref ? 1 : 0};
+    const long long vals[8] = {plan->t8, plan->t8, plan->ta, plan->o8, (long long)plan->tiles.size(), plan->ncta, plan->pblk,
+                               plan->ref ? 1 : (plan->general ? 2 : 0)};
     for (int i = 0; i < n && i < 8; ++i)
         if (info) info[i] = vals[i];
     return 8;

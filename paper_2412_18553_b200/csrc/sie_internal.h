@@ -17,6 +17,7 @@ struct GemmOut {
     int valid_inner;       // column valid iff rem < valid_inner
     long long stride_outer;  // offset = outer * stride_outer + rem
     long long n_lin_total;   // column valid iff n_lin < n_lin_total
+    int accumulate;          // 1: C += (read-modify-write; every element has one owner per launch), 0: C =
 };
 // One GEMM of a grouped launch: C[m][n] = sum_k A[m][k] * Bop[n][k], K-major operands (transform.cu)
 struct alignas(128) XJob {
@@ -27,6 +28,8 @@ struct alignas(128) XJob {
     long long n_total;      // valid flat columns n
     int nao;                // packed mode: n = P * nao + nu
     int M, m8, m_tiles, n_tiles, kblocks;
+    int k0_blocks;          // first K-block of this job (split-K jobs share their tensor maps)
+    int b_c1_off, b_c1_mul, b_c2_mul;  // TMA mode: N-tile nb of Bop sits at coordinates (k, b_c1_off + nb * b_c1_mul, nb * b_c2_mul)
     int tile_begin;         // global index of this job's first tile (tiles of a job: m fastest)
     GemmOut out;
 };
@@ -72,9 +75,25 @@ struct ReduceCluster {             // per cluster, device array
     double* E_out;                 // 1
     double* G_out;                 // [o][o] or nullptr
     int o, o8, nslots;
-    int mode;                      // 0: G_out = G, E_out = sum P o G^T; 1: G_out = 2 delta - 2 Gamma, E_out = its trace
+    int mode;                      // 0: G_out = G, E_out = sum P o G^T; 1: G_out = 2 delta - 2 Gamma, E_out = its trace;
+                                   // 2: G_out = 2 * sum (virtual block gamma_ab, Eq. S17), E_out = its trace
 };
 int launch_reduce(const ReduceCluster* d_rc, int ncluster, cudaStream_t st);
+
+// ---- general.cu --------------------------------------------------------------------------------
+// Any-size pair stage (nocc > 128, and gamma_vir at every size): slab GEMM -> combine -> split-K Gram GEMM per occupied block.
+struct GeneralGeom {
+    int Kb, ldc;                 // occupied block (power of two), leading dimension of a slab row = ceil8(v * Kb)
+    int nsplit_occ, nsplit_vir;  // K splits (= partial slots) of the Gram GEMM of the occupied / virtual block
+    int max_jobs;                // job descriptors per occupied block
+    bool ok;                     // false: one slab would exceed 4 GB (sizes beyond this route)
+    size_t slab_bytes, slots_bytes;
+};
+GeneralGeom general_geom(int o, int v, int num_sms);
+size_t general_scratch_bytes(const GeneralGeom& g, int o);
+// mode 0: G (energy path), 1: Gamma_occ, 2: gamma_vir / 2.  Partial results in slots [*nslots][n*n], n = o (modes 0, 1) or v.
+int general_pair(const GeneralGeom& g, const double* Bmat, int o, int v, int naux, int naux_ld, const double* e_occ, const double* e_vir,
+                 int mode, unsigned char* scratch, double* slots, int* nslots, int num_sms, cudaStream_t st);
 
 // ---- ref_kernels.cu ----------------------------------------------------------------------------
 // Simple FP64-FMA kernels following the definition step by step (any nocc). B layout [v][o][naux_ld].

@@ -176,9 +176,10 @@ __global__ void __launch_bounds__(XG_THREADS, 1) xform_gemm_kernel(const XJob* _
                     mbar_arrive_expect_tx(&full[ps.stage], (uint32_t)(XG_NSUB * (rowsA + XG_TN) * XG_KB * 8));
 #pragma unroll
                     for (int u = 0; u < XG_NSUB; ++u) {
-                        const int kk = (ks * XG_NSUB + u) * XG_KB;
+                        const int kk = (J->k0_blocks + ks * XG_NSUB + u) * XG_KB;
                         tma_load_3d(s + u * XG_SUB_DOUBLES, &J->mapA, &full[ps.stage], kk, mb * rowsA, 0);
-                        tma_load_3d(s + u * XG_SUB_DOUBLES + XG_TMMAX * XG_KB, &J->mapB, &full[ps.stage], kk, nb * XG_TN, 0);
+                        tma_load_3d(s + u * XG_SUB_DOUBLES + XG_TMMAX * XG_KB, &J->mapB, &full[ps.stage], kk, J->b_c1_off + nb * J->b_c1_mul,
+                                    nb * J->b_c2_mul);
                     }
                     ps.advance<XG_STAGES>();
                 }
@@ -221,7 +222,10 @@ __global__ void __launch_bounds__(XG_THREADS, 1) xform_gemm_kernel(const XJob* _
                 const int m = mb * 8 * m8 + row0 + 8 * i + g;
                 if (m >= out.M) continue;
                 double* p = out.base + (long long)m * out.ld_m;
-                if (ok0 && ok1 && off1 == off0 + 1 && ((reinterpret_cast<uintptr_t>(p + off0) & 15) == 0)) {
+                if (out.accumulate) {
+                    if (ok0) p[off0] += acc[i][j][0];
+                    if (ok1) p[off1] += acc[i][j][1];
+                } else if (ok0 && ok1 && off1 == off0 + 1 && ((reinterpret_cast<uintptr_t>(p + off0) & 15) == 0)) {
                     *reinterpret_cast<double2*>(p + off0) = make_double2(acc[i][j][0], acc[i][j][1]);
                 } else {
                     if (ok0) p[off0] = acc[i][j][0];

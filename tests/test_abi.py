@@ -62,13 +62,27 @@ def test_plan_is_host_only_and_reports_workspace():
         info = sie.sie_dfmp2_plan_info(plan)
         assert (info["ta"], info["TM"], info["TN"]) == (ta, t8, t8), (o, info)
         sie.sie_dfmp2_destroy(plan)
-    # nocc > 128 -> reference kernels
-    plan, _ = sie.sie_dfmp2_plan(400, 130, 200, 300)
+    # nocc > 128 -> the general (slab / Gram) route; SIE_FLAG_REFERENCE -> the simple kernels; the route is reported, never silent
+    plan, ws0 = sie.sie_dfmp2_plan(400, 130, 200, 300)
+    info = sie.sie_dfmp2_plan_info(plan)
+    assert info["general"] == 1 and info["reference"] == 0 and info["route"] == 2
+    sie.sie_dfmp2_destroy(plan)
+    plan, _ = sie.sie_dfmp2_plan(400, 130, 200, 300, 0, binding.SIE_FLAG_REFERENCE)
     assert sie.sie_dfmp2_plan_info(plan)["reference"] == 1
     sie.sie_dfmp2_destroy(plan)
+    # SIE_FLAG_RDM_VIR reserves the three amplitude slabs of sie_dfmp2_rdm_vir
+    plan, ws1 = sie.sie_dfmp2_plan(300, 30, 270, 1200)
+    sie.sie_dfmp2_destroy(plan)
+    plan, ws2 = sie.sie_dfmp2_plan(300, 30, 270, 1200, 0, binding.SIE_FLAG_RDM_VIR)
+    sie.sie_dfmp2_destroy(plan)
+    assert ws2 >= ws1 + 3 * 30 * 270 * 270 * 8
+    # an amplitude slab beyond 4 GB is refused at plan time (sizes of the out-of-core NEXT-2 row)
+    with pytest.raises(sie.SieError) as ei:
+        sie.sie_dfmp2_plan(7000, 454, 5903, 19000)
+    assert ei.value.status == binding.SIE_EINVAL
 
 
-@pytest.mark.parametrize("args", [(0, 1, 1, 1), (10, 0, 5, 5), (10, 5, 0, 5), (10, 5, 5, 0), (9, 5, 5, 5), (10, 5, 5, 5, -1), (10, 5, 5, 5, 0, 64)])
+@pytest.mark.parametrize("args", [(0, 1, 1, 1), (10, 0, 5, 5), (10, 5, 0, 5), (10, 5, 5, 0), (9, 5, 5, 5), (10, 5, 5, 5, -1), (10, 5, 5, 5, 0, 128)])
 def test_plan_rejects_bad_sizes(args):
     with pytest.raises(sie.SieError) as ei:
         sie.sie_dfmp2_plan(*args)

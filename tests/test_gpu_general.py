@@ -1,0 +1,142 @@
+"""GPU parity of the any-size pair-stage route (csrc/general.cu) against the CPU oracle, element by element:
+
+  * nocc > 128 — the environment-occupied x impurity-virtual sub-space shape of PAPER.md Eq. S13 (L338): energy, G and
+    gamma_occ (Eq. S18) through the slab GEMM / amplitude pass / split-K Gram GEMM route (plan_info route == 2);
+  * gamma_vir (Eq. S17) at every size (small-occ x large-vir of Eq. S14 and the mirrored shape), plans created
+    with SIE_FLAG_RDM_VIR;
+  * Tr gamma_occ + Tr gamma_vir = 2 nocc on the GPU, call-order / flag errors, a batch that mixes routes.
+
+Tolerances as everywhere: E 1e-10 relative; matrices 1e-11 * max(1, max|oracle|) (inputs scale="std" unless stated).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2412_18553_b200 as sie
+from paper_2412_18553_b200 import binding
+from workloads import ClusterSpec, config_specs, make_cluster
+
+pytestmark = pytest.mark.gpu
+ATOL = 1e-11
+
+
+def _cu(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _solve(spec, flags=0, blocks=None, want=("E", "occ", "vir")):
+    x = make_cluster(spec)
+    s = sie.ClusterSolver(spec.nao, spec.nocc, spec.nvir, spec.naux, flags=flags)
+    info = s.info()
+    C_occ, C_vir = _cu(x.C_occ), _cu(x.C_vir)
+    for p0, p1 in (blocks or [(0, spec.naux)]):
+        s.transform(C_occ, C_vir, _cu(x.L_block(p0, p1, threads=4)), p0, p1)
+    e_occ, e_vir = _cu(x.e_occ), _cu(x.e_vir)
+    out = {}
+    if "E" in want:
+        E, G = s.energy(e_occ, e_vir, None if spec.rank <= 0 else _cu(x.P_frag))
+        out["E"], out["G"] = E, G
+    if "occ" in want:
+        out["occ"], out["tr_occ"] = s.rdm_occ(e_occ, e_vir)
+    if "vir" in want:
+        out["vir"], out["tr_vir"] = s.rdm_vir(e_occ, e_vir)
+    torch.cuda.synchronize()
+    out = {k: (v.cpu().numpy() if v.numel() > 1 else float(v.cpu()[0])) for k, v in out.items()}
+    s.close()
+    return x, info, out
+
+
+def _close(got, ref):
+    scale = max(1.0, float(np.max(np.abs(ref))))
+    err = float(np.max(np.abs(got - ref)))
+    assert err <= ATOL * scale, (err, scale)
+
+
+def _oracle_B(x):
+    return oracle.transform(x.C_occ, x.C_vir, x.L_packed(threads=4))
+
+
+@pytest.mark.parametrize("o,v,extra,naux,rank", [(130, 20, 0, 24, 10), (200, 24, 0, 64, 0), (144, 40, 5, 91, 30), (257, 9, 0, 40, 7),
+                                                  (136, 64, 0, 33, 17)])
+def test_general_route_energy_G_and_both_rdm_blocks(o, v, extra, naux, rank):
+    spec = ClusterSpec(80, o, o + v + extra, o, v, naux, rank, "std")
+    cuts = sorted({0, naux // 2, naux})
+    blocks = [(cuts[i], cuts[i + 1]) for i in range(len(cuts) - 1)][::-1]
+    x, info, out = _solve(spec, flags=binding.SIE_FLAG_RDM_VIR, blocks=blocks)
+    assert info["general"] == 1 and info["reference"] == 0
+    B = _oracle_B(x)
+    Gor = oracle.pair_G(B, x.e_occ, x.e_vir)
+    Eor = oracle.trace(None if rank <= 0 else x.P_frag, Gor)
+    assert abs(out["E"] - Eor) <= 1e-10 * abs(Eor), (out["E"], Eor)
+    _close(out["G"], Gor)
+    gocc, gvir = oracle.rdm_occ(B, x.e_occ, x.e_vir), oracle.rdm_vir(B, x.e_occ, x.e_vir)
+    _close(out["occ"], gocc)
+    _close(out["vir"], gvir)
+    assert abs(out["tr_occ"] - np.trace(gocc)) <= 1e-10 * abs(np.trace(gocc))
+    assert abs(out["tr_vir"] - np.trace(gvir)) <= 1e-10 * max(1.0, abs(np.trace(gvir)))
+    assert abs(out["tr_occ"] + out["tr_vir"] - 2.0 * o) <= 1e-10 * 2.0 * o  # electron count conserved (pin of O9, on the GPU)
+
+
+@pytest.mark.parametrize("scale", ["var", "std"])
+def test_rdm_vir_config0(scale):
+    spec = config_specs(0, scale)[0]
+    x, info, out = _solve(spec, flags=binding.SIE_FLAG_RDM_VIR)
+    assert info["general"] == 0  # fused route for the energy, general route only for gamma_vir
+    B = _oracle_B(x)
+    _close(out["vir"], oracle.rdm_vir(B, x.e_occ, x.e_vir))
+    _close(out["occ"], oracle.rdm_occ(B, x.e_occ, x.e_vir))
+    Gor = oracle.pair_G(B, x.e_occ, x.e_vir)
+    assert abs(out["E"] - oracle.trace(x.P_frag, Gor)) <= 1e-10 * abs(oracle.trace(x.P_frag, Gor))
+
+
+@pytest.mark.parametrize("o,v,extra,naux", [(4, 150, 0, 60), (30, 100, 0, 200), (17, 129, 3, 75), (1, 40, 0, 16), (64, 65, 0, 50), (9, 8, 0, 5)])
+def test_rdm_vir_small_occ_large_vir_shapes(o, v, extra, naux):
+    """The impurity-occupied x environment-virtual shape of Eq. S14 and ragged sizes (v not a multiple of 8 or 128,
+    occupied blocks with a ragged tail, nocc + nvir < nao)."""
+    spec = ClusterSpec(81, o, o + v + extra, o, v, naux, 0, "std")
+    x, info, out = _solve(spec, flags=binding.SIE_FLAG_RDM_VIR, want=("vir", "occ"))
+    B = _oracle_B(x)
+    gvir = oracle.rdm_vir(B, x.e_occ, x.e_vir)
+    _close(out["vir"], gvir)
+    assert np.max(np.abs(out["vir"] - out["vir"].T)) <= ATOL * max(1.0, float(np.max(np.abs(gvir))))
+    assert abs(out["tr_occ"] + out["tr_vir"] - 2.0 * o) <= 1e-10 * 2.0 * o
+
+
+def test_rdm_vir_needs_the_plan_flag_and_host_io_works():
+    spec = ClusterSpec(82, 0, 50, 6, 44, 30, 0, "std")
+    x = make_cluster(spec)
+    s = sie.ClusterSolver(spec.nao, spec.nocc, spec.nvir, spec.naux)  # no SIE_FLAG_RDM_VIR
+    s.transform(_cu(x.C_occ), _cu(x.C_vir), _cu(x.L_packed()), 0, spec.naux)
+    with pytest.raises(sie.SieError) as ei:
+        s.rdm_vir(_cu(x.e_occ), _cu(x.e_vir))
+    assert ei.value.status == binding.SIE_ESTATE
+    s.close()
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
+    h = sie.ClusterSolver(spec.nao, spec.nocc, spec.nvir, spec.naux, flags=binding.SIE_FLAG_HOST_IO | binding.SIE_FLAG_RDM_VIR)
+    h.transform(pin(x.C_occ), pin(x.C_vir), pin(x.L_packed()), 0, spec.naux)
+    g, tr = h.rdm_vir(pin(x.e_occ), pin(x.e_vir))
+    gor = oracle.rdm_vir(_oracle_B(x), x.e_occ, x.e_vir)
+    _close(g.numpy(), gor)
+    assert abs(float(tr[0]) - np.trace(gor)) <= 1e-10 * max(1.0, abs(np.trace(gor)))
+    h.close()
+
+
+def test_batch_mixes_fused_and_general_clusters():
+    shapes = [(16, 40, 50), (150, 12, 40), (33, 64, 72), (129, 20, 24)]
+    specs = [ClusterSpec(83, k, o + v, o, v, naux, max(1, o // 4), "std") for k, (o, v, naux) in enumerate(shapes)]
+    cl, xs = [], []
+    for sp in specs:
+        x = make_cluster(sp)
+        xs.append(x)
+        cl.append(dict(nao=sp.nao, nocc=sp.nocc, nvir=sp.nvir, naux=sp.naux, C_occ=_cu(x.C_occ), C_vir=_cu(x.C_vir), L_packed=_cu(x.L_packed()),
+                       e_occ=_cu(x.e_occ), e_vir=_cu(x.e_vir), P_frag=_cu(x.P_frag), E_out=torch.zeros(1, dtype=torch.float64, device="cuda"),
+                       G_out=torch.zeros(sp.nocc, sp.nocc, dtype=torch.float64, device="cuda")))
+    ws = sie.alloc_workspace(sie.sie_dfmp2_batch_query(cl))
+    sie.sie_dfmp2_batch(cl, ws)
+    torch.cuda.synchronize()
+    for sp, x, c in zip(specs, xs, cl):
+        Gor = oracle.pair_G(_oracle_B(x), x.e_occ, x.e_vir)
+        Eor = oracle.trace(x.P_frag, Gor)
+        assert abs(float(c["E_out"].cpu()[0]) - Eor) <= 1e-10 * abs(Eor), sp
+        _close(c["G_out"].cpu().numpy(), Gor)

@@ -123,7 +123,7 @@ def test_ragged_shapes(nocc, nvir, extra, naux):
     check(spec, E, G)
 
 
-def test_nocc_above_128_uses_reference_path():
+def test_nocc_above_128_uses_general_route():
     spec = ClusterSpec(51, 0, 130 + 20, 130, 20, 24, 10, "std")
     E, G = gpu_run(spec)
     check(spec, E, G)

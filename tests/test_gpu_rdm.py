@@ -67,7 +67,7 @@ def test_ragged_shapes(nocc, nvir, extra, naux):
 
 def test_host_io_and_nocc_above_128():
     _check(ClusterSpec(56, 0, 24 + 60, 24, 60, 50, 1, "std"), binding.SIE_FLAG_HOST_IO)
-    _check(ClusterSpec(56, 1, 130 + 20, 130, 20, 24, 1, "std"))  # reference kernels
+    _check(ClusterSpec(56, 1, 130 + 20, 130, 20, 24, 1, "std"))  # general route (nocc > 128)
 
 
 def test_closed_form_o1_v1_on_gpu():
