@@ -418,28 +418,37 @@ class GpuBench:
 
         m["next1"] = None
         if want_rdm and len(specs) == 1:
+            # NEXT-1: both blocks of the MP2 1-RDM on the same transformed B: gamma_occ (fused kernel in amplitude mode, or
+            # the general route for nocc > 128) and gamma_vir (general route), each timed as a whole call
             s0, d0 = specs[0], devc[0]
-            plan, nb = sie.sie_dfmp2_plan(s0.nao, s0.nocc, s0.nvir, s0.naux, 0, 0)
+            plan, nb = sie.sie_dfmp2_plan(s0.nao, s0.nocc, s0.nvir, s0.naux, 0, sie.SIE_FLAG_RDM_VIR)
+            route = sie.sie_dfmp2_plan_info(plan)["route"]
             ws1 = sie.alloc_workspace(nb, dev)
             sie.sie_dfmp2_transform(plan, ws1, d0["C_occ"], d0["C_vir"], d0["L_packed"], 0, s0.naux)
-            gam = torch.zeros(s0.nocc, s0.nocc, dtype=torch.float64, device=dev)
-            tr = torch.zeros(1, dtype=torch.float64, device=dev)
-            for _ in range(max(1, min(warmup, 2))):
-                sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
-            torch.cuda.synchronize()
-            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            reps = max(1, min(steps, 3))
-            ev0.record()
-            for _ in range(reps):
-                sie.sie_dfmp2_rdm_occ(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
-            ev1.record()
-            torch.cuda.synchronize()
-            ms_rdm = ev0.elapsed_time(ev1) / reps
-            f_rdm = alg_flops(s0)["pair_kernel"]  # same contraction count: SYRK of B plus two o^3 products per virtual pair
-            m["next1"] = {"call": "sie_dfmp2_rdm_occ", "ms": ms_rdm, "tflops": f_rdm / (ms_rdm * 1e-3) * 1e-12,
-                          "trace_gamma": float(tr.cpu()[0]), "algorithmic_flops": f_rdm, "includes": "pair kernel (amplitude mode) + reduce"}
+            o_, v_, x_ = s0.nocc, s0.nvir, s0.naux
+            m["next1"] = {"pair_route": ("fused", "reference", "general")[route]}
+            for name_, fn, n_, f_alg in (
+                    ("rdm_occ", sie.sie_dfmp2_rdm_occ, o_, alg_flops(s0)["pair_kernel"]),
+                    ("rdm_vir", sie.sie_dfmp2_rdm_vir, v_, 1.0 * o_ * o_ * v_ * (v_ + 1) * x_ + 2.0 * o_ * o_ * v_ ** 3)):
+                gam = torch.zeros(n_, n_, dtype=torch.float64, device=dev)
+                tr = torch.zeros(1, dtype=torch.float64, device=dev)
+                for _ in range(max(1, min(warmup, 2))):
+                    fn(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
+                torch.cuda.synchronize()
+                ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                reps = max(1, min(steps, 3))
+                ev0.record()
+                for _ in range(reps):
+                    fn(plan, ws1, d0["e_occ"], d0["e_vir"], gam, tr)
+                ev1.record()
+                torch.cuda.synchronize()
+                ms_ = ev0.elapsed_time(ev1) / reps
+                # algorithmic flops: SYRK minimum of the pair integrals + the second-level contraction (2 o^3 v^2 for the
+                # occupied block, 2 o^2 v^3 for the virtual block)
+                m["next1"][name_] = {"ms": ms_, "tflops": f_alg / (ms_ * 1e-3) * 1e-12, "trace": float(tr.cpu()[0]), "algorithmic_flops": f_alg}
+                del gam
             sie.sie_dfmp2_destroy(plan)
-            del ws1, gam
+            del ws1
             torch.cuda.empty_cache()
 
         m["e2e"] = None
@@ -562,8 +571,9 @@ def run_gpu(args) -> None:
             "workspace_bytes": m["ws_bytes"], "input_gen_s": m["t_gen"],
         }
         if m["next1"] is not None:
-            m["next1"]["frac_of_fp64_peak"] = m["next1"]["tflops"] / gb.peak if gb.peak else None
-            line["next1_rdm_occ"] = m["next1"]
+            for k_ in ("rdm_occ", "rdm_vir"):
+                m["next1"][k_]["frac_of_fp64_peak"] = m["next1"][k_]["tflops"] / gb.peak if gb.peak else None
+            line["next1_rdm"] = m["next1"]
         if batch is not None:
             line["batch"] = batch
             line["sweep"] = sweep
@@ -651,7 +661,7 @@ def main() -> None:
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU oracle leg")
     ap.add_argument("--no-extras", dest="extras", action="store_false",
                     help="skip the time-boxed config-2 batch and config-4 sweep sub-objects of the default config-3 line")
-    ap.add_argument("--rdm", action="store_true", help="also time sie_dfmp2_rdm_occ (NEXT-1: occupied MP2 1-RDM block) on the same B")
+    ap.add_argument("--rdm", action="store_true", help="also time sie_dfmp2_rdm_occ and sie_dfmp2_rdm_vir (NEXT-1: both MP2 1-RDM blocks) on the same B")
     ap.add_argument("--streamed", action="store_true", help="feed the packed integrals in aux blocks generated on the fly "
                                                              "(sweep points that do not fit in HBM; not a bench line)")
     ap.add_argument("--stream-gb", type=float, default=8.0, help="size of one streamed aux block in GB")
