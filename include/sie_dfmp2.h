@@ -127,7 +127,11 @@ int sie_dfmp2_rdm_vir(sie_dfmp2_plan_t plan, void* workspace, const double* e_oc
  *    scheduled submission: per-cluster transforms, then ONE persistent pair kernel whose CTAs walk a
  *    static, cost-balanced list of (cluster, tile) work items, then one reduction launch (step A7).
  *      clusters: HOST array of descriptors (pointers device or host per SIE_FLAG_HOST_IO).
- *      workspace_bytes == 0 or workspace == NULL: query only, *needed receives the required size.
+ *      workspace_bytes == 0 or workspace == NULL: query only, *needed receives the required size (make the query with the
+ *      descriptors of the call, L_packed pointers included: the layout depends on which clusters share integrals).
+ *    Shared integrals (device pointers): clusters of one system are different orbital sets over the SAME (P|mu nu)
+ *    (PAPER.md L95).  Batch members that pass the same L_packed pointer with the same nao and naux are transformed
+ *    together — their C_occ columns are stacked into one A1 GEMM — so the integrals are read once for all of them.
  *    With device pointers the transforms of ALL clusters run as one grouped launch per stage (coefficient transposes,
  *    A1 on the packed integrals, A2) and everything is enqueued on `cuda_stream`; with host pointers the clusters'
  *    integrals pass through one staging ring on an internal copy stream, cluster by cluster.

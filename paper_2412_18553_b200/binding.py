@@ -244,10 +244,14 @@ def _descs(clusters: Sequence[dict], host: bool) -> ctypes.Array:
 
 
 def sie_dfmp2_batch_query(clusters: Sequence[dict], flags: int = 0) -> int:
-    """Workspace bytes needed for this batch (sizes only are read)."""
+    """Workspace bytes needed for this batch.  Sizes are enough; when the L_packed tensors are given too, clusters that
+    share one tensor are laid out as a shared-integral group (never larger than the private layout)."""
     arr = (sie_dfmp2_cluster_t * max(1, len(clusters)))()
+    host = bool(flags & SIE_FLAG_HOST_IO)
     for k, c in enumerate(clusters):
         arr[k].nao, arr[k].nocc, arr[k].nvir, arr[k].naux = c["nao"], c["nocc"], c["nvir"], c["naux"]
+        if c.get("L_packed") is not None:
+            arr[k].L_packed = _ptr(c["L_packed"], host, "L_packed")
     need = ctypes.c_size_t()
     _check(_lib().sie_dfmp2_batch(len(clusters), arr, None, 0, ctypes.byref(need), flags, None), "sie_dfmp2_batch(query)")
     return need.value

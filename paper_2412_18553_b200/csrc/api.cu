@@ -734,6 +734,33 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
         std::vector<sie_dfmp2_plan_s> plans(ncluster);
         Carver c;
         std::vector<size_t> off_cl(ncluster), off_io(ncluster);
+        // Clusters of ONE system share their three-index integrals (the SIE access pattern: every cluster is a
+        // different orbital set C over the same (P|mu nu)): members of a batch that pass the same L_packed pointer with the
+        // same nao and naux are transformed together — their C_occ columns are stacked into one A1 GEMM, so (P|mu nu) is
+        // read once for all of them instead of once per cluster.  (Device pointers only.  The workspace layout depends on
+        // the grouping, so a size query must be made with the same descriptors, pointers included, as the call.)
+        struct SharedGroup {
+            std::vector<int> members;
+            std::vector<int> row0;  // first stacked occupied row of each member
+            int o_sum = 0, pblk = 0;
+            size_t off_CoT = 0, off_H = 0;
+        };
+        std::vector<SharedGroup> groups;
+        std::vector<int> group_of(ncluster, -1);
+        std::vector<size_t> off_CvT_shared(ncluster, 0);
+        if (!host && !(flags & SIE_FLAG_REFERENCE)) {
+            for (int k = 0; k < ncluster; ++k) {
+                if (!clusters[k].L_packed || group_of[k] >= 0) continue;
+                SharedGroup g;
+                for (int m = k; m < ncluster; ++m)
+                    if (group_of[m] < 0 && clusters[m].L_packed == clusters[k].L_packed && clusters[m].nao == clusters[k].nao &&
+                        clusters[m].naux == clusters[k].naux)
+                        g.members.push_back(m);
+                if (g.members.size() < 2) continue;
+                for (int m : g.members) group_of[m] = (int)groups.size();
+                groups.push_back(g);
+            }
+        }
         size_t max_CoT = 0, max_CvT = 0, max_H = 0, max_refH = 0, max_refVj = 0, max_stage = 0, ntiles_total = 0, max_jobs1 = 0, group_jobs = 0, max_gen = 0;
         int nfused = 0;
         for (int k = 0; k < ncluster; ++k) {
@@ -741,15 +768,16 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             if (!query && (!cl.C_occ || !cl.C_vir || !cl.L_packed || !cl.e_occ || !cl.e_vir || !cl.E_out)) return SIE_EINVAL;
             sie_dfmp2_plan_s& p = plans[k];
             SIE_TRY(plan_init(p, cl.nao, cl.nocc, cl.nvir, cl.naux, 0, flags & ~(SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_OCC),
-                              host ? CARVE_NONE : CARVE_MEMBER));
+                              (host || group_of[k] >= 0) ? CARVE_NONE : CARVE_MEMBER));
             off_cl[k] = c.take(p.total);
+            if (group_of[k] >= 0) off_CvT_shared[k] = c.take((size_t)p.v * p.nao_ld * 8);
             if (!p.ref) {
                 ++nfused;
                 max_CoT = std::max(max_CoT, (size_t)p.o * p.nao_ld * 8);
                 max_CvT = std::max(max_CvT, (size_t)p.v * p.nao_ld * 8);
                 max_H = std::max(max_H, (size_t)p.o * p.pblk * p.nao_ld * 8);
                 max_jobs1 = std::max(max_jobs1, (size_t)p.max_jobs);
-                group_jobs += 2 * (size_t)((p.naux + p.pblk - 1) / p.pblk);
+                if (group_of[k] < 0) group_jobs += 2 * (size_t)((p.naux + p.pblk - 1) / p.pblk);
                 ntiles_total += p.tiles.size();
             } else {
                 max_refH = std::max(max_refH, (size_t)p.pblk * p.o * p.nao * 8);
@@ -761,6 +789,21 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                 size_t d = (size_t)p.nao * p.o + (size_t)p.nao * p.v + p.o + p.v + 2 * (size_t)p.o * p.o + 2;
                 off_io[k] = c.take(d * 8);
             }
+        }
+        for (SharedGroup& g : groups) {
+            const sie_dfmp2_plan_s& p0 = plans[g.members[0]];
+            for (int m : g.members) {
+                g.row0.push_back(g.o_sum);
+                g.o_sum += plans[m].o;
+            }
+            const size_t per_p = (size_t)g.o_sum * p0.nao_ld * 8;
+            long long pb = std::max<long long>(8, (long long)(((size_t)2 << 30) / per_p));
+            pb = std::min<long long>(pb, (long long)0x7fffffff / std::max(p0.nao, g.o_sum) - 1);
+            if (pb < p0.naux) pb = std::max<long long>(8, pb / 8 * 8);
+            g.pblk = (int)std::min<long long>(pb, p0.naux);
+            g.off_CoT = c.take((size_t)g.o_sum * p0.nao_ld * 8);
+            g.off_H = c.take((size_t)g.o_sum * g.pblk * p0.nao_ld * 8);
+            group_jobs += (size_t)((p0.naux + g.pblk - 1) / g.pblk) * (1 + g.members.size());
         }
         size_t off_CoT = 0, off_CvT = 0, off_H = 0;
         if (host) {
@@ -874,18 +917,30 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
                                        clusters[k].L_packed, true, 0, p.naux, st));
             }
         } else {
-            // one transpose launch, then per round r (the r-th H sub-block of every cluster) ONE A1 and ONE A2 launch
+            // one transpose launch, then per round r (the r-th H sub-block of every cluster / shared group) ONE A1 and ONE A2 launch
             std::vector<TJob> tj;
             int max_rows = 1, max_cols = 1, rounds = 0;
+            std::vector<double*> CvT(ncluster, nullptr);
             for (int k = 0; k < ncluster; ++k) {
                 sie_dfmp2_plan_s& p = plans[k];
                 if (p.ref) continue;
                 unsigned char* wk = ws + off_cl[k];
-                tj.push_back(TJob{dCo[k], reinterpret_cast<double*>(wk + p.off_CoT), p.nao, p.o, p.nao_ld, 0});
-                tj.push_back(TJob{dCv[k], reinterpret_cast<double*>(wk + p.off_CvT), p.nao, p.v, p.nao_ld, 0});
+                double* CoT;
+                if (group_of[k] >= 0) {
+                    const SharedGroup& g = groups[group_of[k]];
+                    const int idx = (int)(std::find(g.members.begin(), g.members.end(), k) - g.members.begin());
+                    CoT = reinterpret_cast<double*>(ws + g.off_CoT) + (size_t)g.row0[idx] * p.nao_ld;
+                    CvT[k] = reinterpret_cast<double*>(ws + off_CvT_shared[k]);
+                    rounds = std::max(rounds, (p.naux + g.pblk - 1) / g.pblk);
+                } else {
+                    CoT = reinterpret_cast<double*>(wk + p.off_CoT);
+                    CvT[k] = reinterpret_cast<double*>(wk + p.off_CvT);
+                    rounds = std::max(rounds, (p.naux + p.pblk - 1) / p.pblk);
+                }
+                tj.push_back(TJob{dCo[k], CoT, p.nao, p.o, p.nao_ld, 0});
+                tj.push_back(TJob{dCv[k], CvT[k], p.nao, p.v, p.nao_ld, 0});
                 max_rows = std::max(max_rows, p.nao);
                 max_cols = std::max(max_cols, std::max(p.o, p.v));
-                rounds = std::max(rounds, (p.naux + p.pblk - 1) / p.pblk);
             }
             if (!tj.empty()) {
                 unsigned char* d = arena + njobs_arena * sizeof(XJob);
@@ -898,20 +953,40 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             for (int r = 0; r < rounds; ++r) {
                 j1.clear();
                 j2.clear();
-                for (int k = 0; k < ncluster; ++k) {
+                XJob J;
+                for (int k = 0; k < ncluster; ++k) {  // clusters with private integrals
                     sie_dfmp2_plan_s& p = plans[k];
-                    if (p.ref) continue;
+                    if (p.ref || group_of[k] >= 0) continue;
                     const int q0 = r * p.pblk;
                     if (q0 >= p.naux) continue;
                     const int pb = std::min(p.pblk, p.naux - q0);
                     unsigned char* wk = ws + off_cl[k];
                     double* H = reinterpret_cast<double*>(wk + p.off_H);
-                    XJob J;
                     SIE_TRY(make_a1_job(J, p, reinterpret_cast<const double*>(wk + p.off_CoT), clusters[k].L_packed + (size_t)q0 * p.npair, pb,
                                         H, 0, pb));
                     j1.push_back(J);
-                    SIE_TRY(make_a2_job(J, p, reinterpret_cast<const double*>(wk + p.off_CvT), H, pb, reinterpret_cast<double*>(wk + p.off_B), q0));
+                    SIE_TRY(make_a2_job(J, p, CvT[k], H, pb, reinterpret_cast<double*>(wk + p.off_B), q0));
                     j2.push_back(J);
+                }
+                for (const SharedGroup& g : groups) {  // shared integrals: one A1 job over the stacked occupied columns
+                    const int k0 = g.members[0];
+                    sie_dfmp2_plan_s pg = plans[k0];  // a copy that stands for the stacked cluster (sizes only)
+                    pg.o = g.o_sum;
+                    const int q0 = r * g.pblk;
+                    if (q0 >= pg.naux) continue;
+                    const int pb = std::min(g.pblk, pg.naux - q0);
+                    double* H = reinterpret_cast<double*>(ws + g.off_H);
+                    SIE_TRY(make_a1_job(J, pg, reinterpret_cast<const double*>(ws + g.off_CoT), clusters[k0].L_packed + (size_t)q0 * pg.npair,
+                                        pb, H, 0, pb));
+                    j1.push_back(J);
+                    for (size_t m = 0; m < g.members.size(); ++m) {
+                        const int k = g.members[m];
+                        sie_dfmp2_plan_s& p = plans[k];
+                        // member rows [row0, row0 + o) of H[i][P][nu] are one contiguous slice
+                        SIE_TRY(make_a2_job(J, p, CvT[k], H + (size_t)g.row0[m] * pb * p.nao_ld, pb,
+                                            reinterpret_cast<double*>(ws + off_cl[k] + p.off_B), q0));
+                        j2.push_back(J);
+                    }
                 }
                 if (used + j1.size() + j2.size() > njobs_arena) return SIE_EINVAL;  // cannot happen: counted above
                 SIE_TRY(launch_jobs(j1, true, arena + used * sizeof(XJob), plans[0].num_sms, prof, ST_T1, st));

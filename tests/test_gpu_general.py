@@ -140,3 +140,37 @@ def test_batch_mixes_fused_and_general_clusters():
         Eor = oracle.trace(x.P_frag, Gor)
         assert abs(float(c["E_out"].cpu()[0]) - Eor) <= 1e-10 * abs(Eor), sp
         _close(c["G_out"].cpu().numpy(), Gor)
+
+
+def test_batch_clusters_sharing_one_integral_tensor():
+    """Clusters of one system: different orbital sets C over the SAME (P|mu nu).  Passing one L_packed
+    tensor for several batch members makes the library transform them together (one A1 GEMM over the stacked occupied
+    columns); results must equal the oracle run on each cluster separately."""
+    nao, naux = 96, 70
+    shapes = [(12, 60), (30, 66), (7, 40), (20, 70)]
+    base = make_cluster(ClusterSpec(84, 99, nao, 8, 8, naux, 0, "std"))
+    Lh = base.L_packed()
+    L = _cu(Lh)
+    cl, xs = [], []
+    for k, (o, v) in enumerate(shapes):
+        sp = ClusterSpec(84, k, nao, o, v, naux, max(1, o // 3), "std")
+        x = make_cluster(sp)
+        xs.append(x)
+        cl.append(dict(nao=nao, nocc=o, nvir=v, naux=naux, C_occ=_cu(x.C_occ), C_vir=_cu(x.C_vir), L_packed=L, e_occ=_cu(x.e_occ),
+                       e_vir=_cu(x.e_vir), P_frag=_cu(x.P_frag), E_out=torch.zeros(1, dtype=torch.float64, device="cuda"),
+                       G_out=torch.zeros(o, o, dtype=torch.float64, device="cuda")))
+    # one extra member with its own integrals in the same batch
+    own = make_cluster(ClusterSpec(84, 50, 40, 6, 30, 33, 2, "std"))
+    cl.append(dict(nao=40, nocc=6, nvir=30, naux=33, C_occ=_cu(own.C_occ), C_vir=_cu(own.C_vir), L_packed=_cu(own.L_packed()),
+                   e_occ=_cu(own.e_occ), e_vir=_cu(own.e_vir), P_frag=_cu(own.P_frag), E_out=torch.zeros(1, dtype=torch.float64, device="cuda"),
+                   G_out=torch.zeros(6, 6, dtype=torch.float64, device="cuda")))
+    ws = sie.alloc_workspace(sie.sie_dfmp2_batch_query(cl))  # the query sees the shared tensor: same layout as the call
+    l0 = sie.launch_count()
+    sie.sie_dfmp2_batch(cl, ws)
+    torch.cuda.synchronize()
+    assert sie.launch_count() - l0 == 5  # transposes, A1, A2, pair, reduce: the whole batch
+    for x, c, Lx in list(zip(xs, cl, [Lh] * 4)) + [(own, cl[-1], own.L_packed())]:
+        Gor = oracle.pair_G(oracle.transform(x.C_occ, x.C_vir, Lx), x.e_occ, x.e_vir)
+        Eor = oracle.trace(x.P_frag, Gor)
+        assert abs(float(c["E_out"].cpu()[0]) - Eor) <= 1e-10 * abs(Eor)
+        _close(c["G_out"].cpu().numpy(), Gor)
