@@ -9,7 +9,7 @@ projector/trace reduction) over one synthetic workload of BASELINE.json:
     config1                          one cluster o=30 v=270 nao=300 naux=1200
     config2                          96 clusters through sie_dfmp2_batch (clusters/s)
     config4:<k>                      sweep point k in 0..3 (o=64, v=256/512/1024/2048)
-    custom:o,v,naux                  one cluster of that shape (nao=o+v): short slices for ncu captures
+    custom:o,v,naux[,rank]           one cluster of that shape (nao=o+v): short slices for ncu captures
 `value` is algorithmic FP64 TFLOP/s (minimum flops of the method / device time) with the inputs resident in HBM;
 `e2e` is the same metric through the C ABI with HOST (pinned) buffers, H2D/D2H inside the timed region.
 N > 1 (torchrun): independent replicas, one cluster (batch) per GPU, no data-path collective ("replicas only").
@@ -86,8 +86,9 @@ def exec_pair_flops(s: ClusterSpec, info: dict) -> float:
 def workload_specs(name: str, rank: int):
     """Cluster list of one replica. Replica r > 0 draws its own clusters (cluster_id shifted by 1000 r)."""
     if name.startswith("custom:"):  # profiling slices, e.g. custom:120,216,4800 = a 1/5-virtuals slice of config 3
-        o, v, naux = (int(x) for x in name.split(":")[1].split(",")[:3])
-        specs = [ClusterSpec(9, 0, o + v, o, v, naux, max(1, o // 2))]
+        f = [int(x) for x in name.split(":")[1].split(",")]
+        o, v, naux = f[:3]
+        specs = [ClusterSpec(9, 0, o + v, o, v, naux, f[3] if len(f) > 3 else max(1, o // 2))]  # optional 4th field: projector rank
     elif name.startswith("config4"):
         k = int(name.split(":")[1]) if ":" in name else 2
         specs = [config_specs(4)[2 * k]]
@@ -447,6 +448,28 @@ class GpuBench:
                 # occupied block, 2 o^2 v^3 for the virtual block)
                 m["next1"][name_] = {"ms": ms_, "tflops": f_alg / (ms_ * 1e-3) * 1e-12, "trace": float(tr.cpu()[0]), "algorithmic_flops": f_alg}
                 del gam
+            # NEXT-3: energy only, projector in factored form Q Q^T (project-first epilogue for rank <= 32), against the
+            # G-path energy with P = Q Q^T on the same B
+            if route == 0 and s0.rank > 0:
+                Qd = torch.from_numpy(np.ascontiguousarray(make_cluster(s0).Q_frag)).to(dev)
+                Pd = (Qd @ Qd.T).contiguous()
+                E1 = torch.zeros(1, dtype=torch.float64, device=dev)
+                G1 = torch.zeros(o_, o_, dtype=torch.float64, device=dev)
+                res = {}
+                for name_, call in (("energy_lowrank", lambda: sie.sie_dfmp2_energy_lowrank(plan, ws1, d0["e_occ"], d0["e_vir"], Qd, E1)),
+                                    ("energy_G_path", lambda: sie.sie_dfmp2_energy(plan, ws1, d0["e_occ"], d0["e_vir"], Pd, E1, G1))):
+                    for _ in range(2):
+                        call()
+                    torch.cuda.synchronize()
+                    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    reps = max(1, min(steps, 3))
+                    ev0.record()
+                    for _ in range(reps):
+                        call()
+                    ev1.record()
+                    torch.cuda.synchronize()
+                    res[name_] = {"ms": ev0.elapsed_time(ev1) / reps, "E_frag": float(E1.cpu()[0])}
+                m["next1"]["next3_lowrank"] = dict(res, rank=s0.rank)
             sie.sie_dfmp2_destroy(plan)
             del ws1
             torch.cuda.empty_cache()

@@ -97,6 +97,18 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
                      const double* P_frag, double* E_out, double* G_out, void* cuda_stream);
 
 /*
+ * 3a. sie_dfmp2_energy_lowrank — NEXT-3, "project first" (PAPER.md Eq. S33; fragment projector C^f = sum_f C_if C_i'f,
+ *    Eq. S45): the fragment energy for a projector given in factored form, P_frag = Q Q^T with Q [nocc][r] row-major
+ *    (the r fragment orbitals in the cluster's occupied basis), when G itself is not wanted:  E_frag = Tr(Q Q^T G).
+ *    For r <= 32 the fused kernel contracts every (ia|jb) block with Q^T first — four r x o x o tensor-core products per
+ *    virtual pair instead of two o x o x o ones, and no partial-G slots; above that it forms P and takes the G path.
+ *    Same value as sie_dfmp2_energy(P_frag = Q Q^T) up to rounding order.  Fused route only (nocc <= 128;
+ *    SIE_EUNSUPPORTED otherwise).  Pointers device or host per SIE_FLAG_HOST_IO; call order and errors as sie_dfmp2_energy.
+ */
+int sie_dfmp2_energy_lowrank(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir,
+                             const double* Q, int r, double* E_out, void* cuda_stream);
+
+/*
  * 3b. sie_dfmp2_rdm_occ — NEXT-1: occupied block of the MP2 one-particle reduced density matrix of the
  *    cluster, PAPER.md Eq. S18 (L357) with the amplitudes of Eq. S15-S16 (L348-L351):
  *        gamma_ij = 2 delta_ij - 2 sum_k sum_ab t_ik^ab (2 t_jk^ab - t_jk^ba),   t_ik^ab = (ia|kb) / (e_i + e_k - e_a - e_b)

@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     sie_dfmp2_batch_query,
     sie_dfmp2_destroy,
     sie_dfmp2_energy,
+    sie_dfmp2_energy_lowrank,
     sie_dfmp2_rdm_occ,
     sie_dfmp2_rdm_vir,
     sie_dfmp2_plan,

@@ -22,6 +22,7 @@ EXPORTS = (
     "sie_dfmp2_plan",
     "sie_dfmp2_transform",
     "sie_dfmp2_energy",
+    "sie_dfmp2_energy_lowrank",
     "sie_dfmp2_rdm_occ",
     "sie_dfmp2_rdm_vir",
     "sie_dfmp2_batch",
@@ -85,6 +86,8 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_energy.restype = ci
         L.sie_dfmp2_rdm_occ.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.sie_dfmp2_rdm_occ.restype = ci
+        L.sie_dfmp2_energy_lowrank.argtypes = [vp, vp, vp, vp, vp, ci, vp, vp]
+        L.sie_dfmp2_energy_lowrank.restype = ci
         L.sie_dfmp2_rdm_vir.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.sie_dfmp2_rdm_vir.restype = ci
         L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
@@ -163,6 +166,18 @@ def sie_dfmp2_rdm_occ(plan: int, workspace: torch.Tensor, e_occ, e_vir, gamma_ou
             plan, workspace.data_ptr(), _ptr(e_occ, host, "e_occ"), _ptr(e_vir, host, "e_vir"), _ptr(gamma_out, host, "gamma_out"),
             _ptr(trace_out, host, "trace_out"), _stream_ptr(stream)),
         "sie_dfmp2_rdm_occ",
+    )
+
+
+def sie_dfmp2_energy_lowrank(plan: int, workspace: torch.Tensor, e_occ, e_vir, Q, E_out, *, host=False, stream=None) -> None:
+    """E_frag = Tr(Q Q^T G) for a factored projector Q [nocc][r] (PAPER.md Eq. S33/S45); marshalling only."""
+    if Q.dim() != 2:
+        raise TypeError("Q: need a [nocc][r] matrix")
+    _check(
+        _lib().sie_dfmp2_energy_lowrank(
+            plan, workspace.data_ptr(), _ptr(e_occ, host, "e_occ"), _ptr(e_vir, host, "e_vir"), _ptr(Q, host, "Q"), int(Q.shape[1]),
+            _ptr(E_out, host, "E_out"), _stream_ptr(stream)),
+        "sie_dfmp2_energy_lowrank",
     )
 
 
@@ -303,6 +318,14 @@ class ClusterSolver:
             E, G = E.pin_memory(), (G.pin_memory() if G is not None else None)
         sie_dfmp2_energy(self.plan, self.workspace, e_occ, e_vir, P_frag, E, G, host=self.host, stream=stream)
         return E, G
+
+    def energy_lowrank(self, e_occ, e_vir, Q, stream=None):
+        """-> E_frag = Tr(Q Q^T G) for a factored projector Q [nocc][r]"""
+        E = torch.empty(1, dtype=torch.float64, device="cpu" if self.host else self.device)
+        if self.host:
+            E = E.pin_memory()
+        sie_dfmp2_energy_lowrank(self.plan, self.workspace, e_occ, e_vir, Q, E, host=self.host, stream=stream)
+        return E
 
     def rdm_occ(self, e_occ, e_vir, stream=None):
         """-> (gamma [nocc][nocc], Tr gamma)"""

@@ -198,7 +198,7 @@ struct sie_dfmp2_plan_s {
     unsigned flags = 0;
     bool ref = false, general = false, fused = true, has_gen = false;
     GeneralGeom gen{};
-    size_t off_gen = 0, off_gslots = 0;
+    size_t off_gen = 0, off_gslots = 0, off_Qt = 0;
     int nao_ld = 0, naux_ld = 0, o8 = 0, ta = 1, t8 = 8, nblk = 0, pblk = 0, cblk = 0, max_jobs = 0, ncta = 0, kp = 1, num_sms = 148;
     size_t npair = 0;
     std::vector<PairTile> tiles;  // cluster field = 0; rewritten when used inside a batch
@@ -323,6 +323,7 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
             p.off_H = c.take((size_t)nocc * p.pblk * p.nao_ld * 8);
             p.off_jobs = c.take((size_t)p.max_jobs * sizeof(XJob) + 2 * sizeof(TJob));
             p.off_desc = c.take(sizeof(PairCluster));
+            p.off_Qt = c.take((size_t)32 * p.o8 * 8 + (size_t)nocc * nocc * 8);  // Q^T of a low-rank projector, and P = Q Q^T
             p.off_tiles = c.take(p.tiles.size() * sizeof(PairTile) + 256);  // + the round-gate counter behind the list
         } else {
             p.off_refH = c.take((size_t)p.pblk * nocc * nao * 8);
@@ -706,6 +707,86 @@ int sie_dfmp2_rdm_occ(sie_dfmp2_plan_t plan, void* workspace, const double* e_oc
                       double* trace_out, void* cuda_stream) {
     if (!gamma_out) return SIE_EINVAL;
     return energy_impl(plan, workspace, e_occ, e_vir, nullptr, trace_out, gamma_out, cuda_stream, 1);
+}
+
+int sie_dfmp2_energy_lowrank(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, const double* Q, int r,
+                             double* E_out, void* cuda_stream) {
+    if (!plan || !workspace || !e_occ || !e_vir || !Q || !E_out || r < 1 || r > plan->o) return SIE_EINVAL;
+    sie_dfmp2_plan_s& p = *plan;
+    if (p.covered_rows != p.naux || p.c_ready_ws != workspace) return SIE_ESTATE;
+    if (!p.fused) return SIE_EUNSUPPORTED;  // general / reference routes: form P = Q Q^T and call sie_dfmp2_energy
+    SIE_TRY(check_device());
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    const bool host = p.flags & SIE_FLAG_HOST_IO;
+    const int o = p.o, v = p.v;
+    const double *de_occ = e_occ, *de_vir = e_vir, *dQ = Q;
+    double* dE = E_out;
+    double* io = reinterpret_cast<double*>(ws + p.off_io);
+    if (host) {
+        if (p.flags & SIE_FLAG_VALIDATE) SIE_TRY(check_gap_host(e_occ, e_vir, o, v));
+        SIE_CUDA(cudaMemcpyAsync(io + p.io_eo, e_occ, (size_t)o * 8, cudaMemcpyHostToDevice, st));
+        SIE_CUDA(cudaMemcpyAsync(io + p.io_ev, e_vir, (size_t)v * 8, cudaMemcpyHostToDevice, st));
+        SIE_CUDA(cudaMemcpyAsync(io + p.io_P, Q, (size_t)o * r * 8, cudaMemcpyHostToDevice, st));  // r <= o: fits the P slot
+        de_occ = io + p.io_eo;
+        de_vir = io + p.io_ev;
+        dQ = io + p.io_P;
+        dE = io + p.io_E;
+    } else if (p.flags & SIE_FLAG_VALIDATE) {
+        std::vector<double> he(o + v);
+        SIE_CUDA(cudaMemcpyAsync(he.data(), e_occ, (size_t)o * 8, cudaMemcpyDeviceToHost, st));
+        SIE_CUDA(cudaMemcpyAsync(he.data() + o, e_vir, (size_t)v * 8, cudaMemcpyDeviceToHost, st));
+        SIE_CUDA(cudaStreamSynchronize(st));
+        SIE_TRY(check_gap_host(he.data(), he.data() + o, o, v));
+    }
+    const double* Bmat = reinterpret_cast<const double*>(ws + p.off_B);
+    double* Qt = reinterpret_cast<double*>(ws + p.off_Qt);
+    double* Pbuf = Qt + (size_t)32 * p.o8;
+    double* gpart = reinterpret_cast<double*>(ws + p.off_gpart);
+    const int r8 = (r + 7) / 8;
+    const bool lowrank = r8 <= 4;
+    ReduceCluster rc{};
+    rc.E_out = dE;
+    PairCluster pc;
+    SIE_TRY(fill_pair_cluster(p, Bmat, de_occ, de_vir, gpart, p.kp, pc));
+    pc.gate = 1;
+    SIE_TRY(launch_lowrank_prep(dQ, o, r, lowrank ? Qt : nullptr, p.o8, r8, lowrank ? nullptr : Pbuf, st));
+    if (lowrank) {  // contract with Q^T first: per-warp partial energies, no G
+        pc.mode = 2;
+        pc.Qt = Qt;
+        pc.r8 = r8;
+        pc.ldq = p.o8;
+        SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)p.ncta * pair_geom().ncons * 8, st));
+        rc.o = 1;
+        rc.o8 = 1;
+        rc.nslots = p.ncta * pair_geom().ncons;
+    } else {        // rank above 32: the o x o x o epilogue is the cheaper one; P = Q Q^T through the G path
+        pc.mode = 0;
+        SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)p.ncta * p.kp * p.o8 * p.o8 * 8, st));
+        rc.P = Pbuf;
+        rc.o = o;
+        rc.o8 = p.o8;
+        rc.nslots = p.ncta * p.kp;
+    }
+    rc.gpart = gpart;
+    SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
+    SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+    SIE_CUDA(cudaMemsetAsync(ws + p.off_tiles + p.tiles.size() * sizeof(PairTile), 0, 256, st));
+    {
+        ProfSpan ps(p.prof, ST_PAIR, st);
+        SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc), reinterpret_cast<const PairTile*>(ws + p.off_tiles),
+                            (int)p.tiles.size(), p.ncta, p.t8, pc.mode, st));
+    }
+    SIE_CUDA(cudaMemcpyAsync(ws + p.off_rc, &rc, sizeof rc, cudaMemcpyHostToDevice, st));
+    {
+        ProfSpan ps(p.prof, ST_REDUCE, st);
+        SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
+    }
+    if (host) {
+        SIE_CUDA(cudaMemcpyAsync(E_out, dE, 8, cudaMemcpyDeviceToHost, st));
+        SIE_CUDA(cudaStreamSynchronize(st));
+    }
+    return SIE_OK;
 }
 
 int sie_dfmp2_rdm_vir(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir, double* gamma_out,

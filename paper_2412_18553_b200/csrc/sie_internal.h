@@ -56,6 +56,8 @@ struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (g
     int t8;                        // tile edge in rows of B: ceil8(ta * o) <= 128
     int gate;                      // 1: producers keep the CTAs of a round in K-lockstep (equal-cost tiles only)
     int mode;                      // 0: G of the energy path; 1: Gamma of the occupied 1-RDM block (amplitudes on both sides)
+    const double* Qt;              // mode 2 (energy only, P_frag = Q Q^T of rank r <= 32): Q^T, zero padded, [8*r8][ldq]
+    int r8, ldq;                   //   gpart then holds per-warp partial energies [ncta][16] instead of G slots
 };
 struct PairTile {                  // 8 bytes
     int cluster;
@@ -66,7 +68,7 @@ struct PairGeom {                  // tile configuration facts for host-side pla
 };
 PairGeom pair_geom();
 size_t pair_smem_bytes();
-// mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma); one mode per launch
+// mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma), 2 energy only with a low-rank projector; one mode per launch
 int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, int mode, cudaStream_t st);
 
 struct ReduceCluster {             // per cluster, device array
@@ -79,6 +81,8 @@ struct ReduceCluster {             // per cluster, device array
                                    // 2: G_out = 2 * sum (virtual block gamma_ab, Eq. S17), E_out = its trace
 };
 int launch_reduce(const ReduceCluster* d_rc, int ncluster, cudaStream_t st);
+// Q [o][r] -> Qt (Q^T zero padded to [8*r8][ldq]) when Qt != nullptr, and P = Q Q^T [o][o] when P != nullptr
+int launch_lowrank_prep(const double* Q, int o, int r, double* Qt, int ldq, int r8, double* P, cudaStream_t st);
 
 // ---- general.cu --------------------------------------------------------------------------------
 // Any-size pair stage (nocc > 128, and gamma_vir at every size): slab GEMM -> combine -> split-K Gram GEMM per occupied block.

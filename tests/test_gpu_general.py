@@ -174,3 +174,44 @@ def test_batch_clusters_sharing_one_integral_tensor():
         Eor = oracle.trace(x.P_frag, Gor)
         assert abs(float(c["E_out"].cpu()[0]) - Eor) <= 1e-10 * abs(Eor)
         _close(c["G_out"].cpu().numpy(), Gor)
+
+
+@pytest.mark.parametrize("o,v,naux,r", [(8, 40, 160, 4), (30, 100, 120, 15), (17, 60, 75, 4), (120, 130, 64, 8), (120, 125, 40, 32),
+                                         (120, 125, 40, 33), (33, 70, 50, 1), (64, 96, 100, 32), (5, 9, 7, 5), (128, 130, 24, 17)])
+def test_energy_lowrank_matches_oracle_trace(o, v, naux, r):
+    """NEXT-3: E_frag = Tr(Q Q^T G) through the project-first epilogue (r <= 32) and its fallback (r > 32)."""
+    spec = ClusterSpec(85, o * 1000 + r, o + v, o, v, naux, r, "std")
+    x = make_cluster(spec)
+    s = sie.ClusterSolver(spec.nao, o, v, naux)
+    s.transform(_cu(x.C_occ), _cu(x.C_vir), _cu(x.L_packed(threads=4)), 0, naux)
+    e_occ, e_vir = _cu(x.e_occ), _cu(x.e_vir)
+    E_lr = s.energy_lowrank(e_occ, e_vir, _cu(x.Q_frag))
+    E_full, _ = s.energy(e_occ, e_vir, _cu(x.P_frag))  # the two entry points share the workspace
+    E_lr2 = s.energy_lowrank(e_occ, e_vir, _cu(x.Q_frag))
+    torch.cuda.synchronize()
+    assert torch.equal(E_lr, E_lr2)  # fixed-order reduction of the per-warp partials
+    Gor = oracle.pair_G(_oracle_B(x), x.e_occ, x.e_vir)
+    Eor = oracle.trace(x.Q_frag @ x.Q_frag.T, Gor)
+    assert abs(float(E_lr.cpu()[0]) - Eor) <= 1e-10 * abs(Eor), (float(E_lr.cpu()[0]), Eor)
+    assert abs(float(E_full.cpu()[0]) - Eor) <= 1e-10 * abs(Eor)
+    s.close()
+
+
+def test_energy_lowrank_host_io_and_unsupported_route():
+    spec = ClusterSpec(85, 7, 60, 10, 50, 40, 3, "std")
+    x = make_cluster(spec)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
+    h = sie.ClusterSolver(spec.nao, spec.nocc, spec.nvir, spec.naux, flags=binding.SIE_FLAG_HOST_IO)
+    h.transform(pin(x.C_occ), pin(x.C_vir), pin(x.L_packed()), 0, spec.naux)
+    E = h.energy_lowrank(pin(x.e_occ), pin(x.e_vir), pin(x.Q_frag))
+    Eor = oracle.trace(x.P_frag, oracle.pair_G(_oracle_B(x), x.e_occ, x.e_vir))
+    assert abs(float(E[0]) - Eor) <= 1e-10 * abs(Eor)
+    h.close()
+    big = ClusterSpec(85, 8, 150, 130, 20, 16, 2, "std")  # general route: not supported, loudly
+    xb = make_cluster(big)
+    g = sie.ClusterSolver(big.nao, big.nocc, big.nvir, big.naux)
+    g.transform(_cu(xb.C_occ), _cu(xb.C_vir), _cu(xb.L_packed()), 0, big.naux)
+    with pytest.raises(sie.SieError) as ei:
+        g.energy_lowrank(_cu(xb.e_occ), _cu(xb.e_vir), _cu(xb.Q_frag))
+    assert ei.value.status == binding.SIE_EUNSUPPORTED
+    g.close()

@@ -77,9 +77,11 @@ class ClusterInputs:
         self.e_occ = _rng(spec, _S_EOCC).uniform(-1.5, -0.3, size=nocc)
         self.e_vir = _rng(spec, _S_EVIR).uniform(0.1, 3.0, size=nvir)
         if spec.rank <= 0:
+            self.Q_frag = np.eye(nocc)  # [nocc][rank]: the fragment orbitals in the cluster's occupied basis
             self.P_frag = np.eye(nocc)
         else:
             q = _orthonormal(_rng(spec, _S_Q), nocc, min(spec.rank, nocc))
+            self.Q_frag = q
             self.P_frag = np.ascontiguousarray(q @ q.T)
 
     @property
