@@ -174,6 +174,33 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
  */
 int sie_dfmp2_plan_reset(sie_dfmp2_plan_t plan);
 
+/*
+ * 5. sie_dfmp2_canonical_* — NEXT-2: closed-shell canonical DF-MP2 correlation energy of a whole system,
+ *        E_MP2 = sum_{ij} sum_{ab} (ia|jb) (2 (ia|jb) - (ib|ja)) / (e_i + e_j - e_a - e_b)       (Eq. S15-S16 with P_frag = I),
+ *    the E_MP2 term of the bath-truncation correction (PAPER.md Eq. S63; Eq. S68; Table S1), for sizes
+ *    where B^P_ia no longer fits in device memory.  B[i][a][P] (occupied-major, aux index contiguous, leading dimension
+ *    ceil8(naux)) lives in a STORE the caller owns: pinned host memory for the out-of-core case, or device memory when it
+ *    fits — any pointer cudaMemcpy understands; *bstore_bytes reports its size.
+ *      plan       host only; occ_block = occupied orbitals per panel of the pair phase (0 = auto: three panels and the
+ *                 (block x nvir)^2 integral block within ~12 GB); reports the device workspace.
+ *      transform  aux rows [p0,p1) of the packed integrals (DEVICE pointer, as sie_dfmp2_transform) -> the store; call until
+ *                 [0,naux) is covered exactly once; C_occ, C_vir DEVICE pointers.
+ *      energy     occupied-block pairs I <= K: panels to the device on an internal copy stream (double-buffered under the
+ *                 GEMM of the pair before), one tensor-core GEMM per pair of blocks, an elementwise pass into CTA-private
+ *                 slots, fixed-order sum; e_occ, e_vir, E_out DEVICE pointers.  SIE_ESTATE before the transform is complete.
+ *      info       [0] occupied block  [1] aux sub-block of the transform  [2] number of occupied blocks  [3] bytes of one panel
+ *    Amplitudes are never stored; the (block x nvir)^2 integral block lives for one pair of blocks.
+ */
+typedef struct sie_dfmp2_canon_s* sie_dfmp2_canon_t;
+int sie_dfmp2_canonical_plan(sie_dfmp2_canon_t* plan, int nao, int nocc, int nvir, int naux, int occ_block,
+                             size_t* workspace_bytes, size_t* bstore_bytes);
+int sie_dfmp2_canonical_transform(sie_dfmp2_canon_t plan, void* workspace, const double* C_occ, const double* C_vir,
+                                  const double* L_packed_block, int p0, int p1, double* B_store, void* cuda_stream);
+int sie_dfmp2_canonical_energy(sie_dfmp2_canon_t plan, void* workspace, const double* e_occ, const double* e_vir,
+                               const double* B_store, double* E_out, void* cuda_stream);
+int sie_dfmp2_canonical_info(sie_dfmp2_canon_t plan, long long* info, int n);
+int sie_dfmp2_canonical_destroy(sie_dfmp2_canon_t plan);
+
 /* Frees the host-side plan (never touches device memory). NULL is allowed. */
 int sie_dfmp2_destroy(sie_dfmp2_plan_t plan);
 

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     SIE_FLAG_RDM_VIR,
     SIE_FLAG_REFERENCE,
     SIE_FLAG_VALIDATE,
+    CanonicalSolver,
     ClusterSolver,
     SieError,
     alloc_workspace,

@@ -27,6 +27,11 @@ EXPORTS = (
     "sie_dfmp2_rdm_vir",
     "sie_dfmp2_batch",
     "sie_dfmp2_plan_reset",
+    "sie_dfmp2_canonical_plan",
+    "sie_dfmp2_canonical_transform",
+    "sie_dfmp2_canonical_energy",
+    "sie_dfmp2_canonical_info",
+    "sie_dfmp2_canonical_destroy",
     "sie_dfmp2_destroy",
     "sie_dfmp2_strerror",
     "sie_dfmp2_last_cuda_error",
@@ -92,6 +97,16 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_rdm_vir.restype = ci
         L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
         L.sie_dfmp2_batch.restype = ci
+        L.sie_dfmp2_canonical_plan.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ctypes.POINTER(ctypes.c_size_t), ctypes.POINTER(ctypes.c_size_t)]
+        L.sie_dfmp2_canonical_plan.restype = ci
+        L.sie_dfmp2_canonical_transform.argtypes = [vp, vp, vp, vp, vp, ci, ci, vp, vp]
+        L.sie_dfmp2_canonical_transform.restype = ci
+        L.sie_dfmp2_canonical_energy.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.sie_dfmp2_canonical_energy.restype = ci
+        L.sie_dfmp2_canonical_info.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong), ci]
+        L.sie_dfmp2_canonical_info.restype = ci
+        L.sie_dfmp2_canonical_destroy.argtypes = [vp]
+        L.sie_dfmp2_canonical_destroy.restype = ci
         L.sie_dfmp2_plan_reset.argtypes = [vp]
         L.sie_dfmp2_plan_reset.restype = ci
         L.sie_dfmp2_destroy.argtypes = [vp]
@@ -282,6 +297,52 @@ def sie_dfmp2_batch(clusters: Sequence[dict], workspace: torch.Tensor, flags: in
                                ctypes.byref(need), flags, _stream_ptr(stream)),
         "sie_dfmp2_batch",
     )
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-2: canonical, out of core
+class CanonicalSolver:
+    """Whole-system canonical DF-MP2 energy (sie_dfmp2_canonical_*).  The B store is a pinned host tensor
+    (``store="host"``, the out-of-core case) or a device tensor (``store="device"``).  Marshalling only."""
+
+    def __init__(self, nao: int, nocc: int, nvir: int, naux: int, occ_block: int = 0, store: str = "host", device="cuda"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2412_18553_b200 needs a CUDA device (B200, sm_100a); there is no CPU path")
+        h, ws, bs = ctypes.c_void_p(), ctypes.c_size_t(), ctypes.c_size_t()
+        _check(_lib().sie_dfmp2_canonical_plan(ctypes.byref(h), nao, nocc, nvir, naux, occ_block, ctypes.byref(ws), ctypes.byref(bs)),
+               "sie_dfmp2_canonical_plan")
+        self.plan, self.workspace_bytes, self.bstore_bytes = h.value, ws.value, bs.value
+        self.workspace = alloc_workspace(self.workspace_bytes, device)
+        n = self.bstore_bytes // 8
+        self.B_store = torch.empty(n, dtype=torch.float64, device=device) if store == "device" else torch.empty(n, dtype=torch.float64).pin_memory()
+        self.device = device
+
+    def info(self) -> dict:
+        buf = (ctypes.c_longlong * 4)()
+        _lib().sie_dfmp2_canonical_info(self.plan, buf, 4)
+        return dict(zip(("occ_block", "aux_subblock", "n_occ_blocks", "panel_bytes"), (int(x) for x in buf)))
+
+    def transform(self, C_occ, C_vir, L_block, p0: int, p1: int, stream=None) -> None:
+        _check(_lib().sie_dfmp2_canonical_transform(self.plan, self.workspace.data_ptr(), _ptr(C_occ, False, "C_occ"), _ptr(C_vir, False, "C_vir"),
+                                                    _ptr(L_block, False, "L_packed_block"), p0, p1, self.B_store.data_ptr(), _stream_ptr(stream)),
+               "sie_dfmp2_canonical_transform")
+
+    def energy(self, e_occ, e_vir, stream=None) -> torch.Tensor:
+        E = torch.empty(1, dtype=torch.float64, device=self.device)
+        _check(_lib().sie_dfmp2_canonical_energy(self.plan, self.workspace.data_ptr(), _ptr(e_occ, False, "e_occ"), _ptr(e_vir, False, "e_vir"),
+                                                 self.B_store.data_ptr(), E.data_ptr(), _stream_ptr(stream)),
+               "sie_dfmp2_canonical_energy")
+        return E
+
+    def close(self) -> None:
+        if self.plan:
+            _lib().sie_dfmp2_canonical_destroy(self.plan)
+        self.plan = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 # ------------------------------------------------------------------------------------------------ convenience

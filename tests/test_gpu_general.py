@@ -215,3 +215,40 @@ def test_energy_lowrank_host_io_and_unsupported_route():
         g.energy_lowrank(_cu(xb.e_occ), _cu(xb.e_vir), _cu(xb.Q_frag))
     assert ei.value.status == binding.SIE_EUNSUPPORTED
     g.close()
+
+
+@pytest.mark.parametrize("o,v,extra,naux,occ_block,store", [(8, 40, 0, 160, 0, "device"), (8, 40, 0, 160, 3, "host"), (37, 50, 4, 61, 8, "host"),
+                                                          (150, 24, 0, 40, 64, "host"), (130, 9, 0, 33, 7, "device"), (5, 130, 0, 20, 2, "host")])
+def test_canonical_out_of_core_energy_matches_oracle(o, v, extra, naux, occ_block, store):
+    """NEXT-2: E_MP2 = sum_ij e_ij (P = I) through the occupied-block-pair route with the B store in pinned host memory
+    (panels streamed back, ragged last block, nocc > 128) or in device memory; the oracle is its pinned P = I case (pin P-2)."""
+    spec = ClusterSpec(86, o * 100 + occ_block, o + v + extra, o, v, naux, 0, "std")
+    x = make_cluster(spec)
+    s = sie.CanonicalSolver(spec.nao, o, v, naux, occ_block=occ_block, store=store)
+    info = s.info()
+    if occ_block:
+        assert info["occ_block"] == min(occ_block, o) and info["n_occ_blocks"] == -(-o // min(occ_block, o))
+    C_occ, C_vir = _cu(x.C_occ), _cu(x.C_vir)
+    cuts = sorted({0, naux // 3, naux})
+    for p0, p1 in [(cuts[i], cuts[i + 1]) for i in range(len(cuts) - 1)][::-1]:  # aux blocks, out of order
+        s.transform(C_occ, C_vir, _cu(x.L_block(p0, p1)), p0, p1)
+    E1 = s.energy(_cu(x.e_occ), _cu(x.e_vir))
+    E2 = s.energy(_cu(x.e_occ), _cu(x.e_vir))
+    torch.cuda.synchronize()
+    assert torch.equal(E1, E2)  # fixed-order slot sums
+    B = _oracle_B(x)
+    Eor = oracle.trace(None, oracle.pair_G(B, x.e_occ, x.e_vir))
+    assert abs(float(E1.cpu()[0]) - Eor) <= 1e-10 * abs(Eor), (float(E1.cpu()[0]), Eor)
+    # the store itself, element by element: B[i][a][P]
+    naux_ld = (naux + 7) // 8 * 8
+    Bs = s.B_store.cpu().numpy().reshape(o, v, naux_ld)[:, :, :naux]
+    assert np.max(np.abs(Bs - B)) <= 1e-13 * max(1.0, float(np.max(np.abs(B))))
+    s.close()
+
+
+def test_canonical_call_order():
+    s = sie.CanonicalSolver(20, 4, 16, 12, store="device")
+    with pytest.raises(sie.SieError) as ei:
+        s.energy(torch.zeros(4, dtype=torch.float64, device="cuda"), torch.ones(16, dtype=torch.float64, device="cuda"))
+    assert ei.value.status == binding.SIE_ESTATE
+    s.close()
