@@ -673,6 +673,66 @@ def run_streamed(args) -> None:
     print(json.dumps(line))
 
 
+def run_canonical(args) -> None:
+    """NEXT-2 (not a bench line): whole-system canonical DF-MP2 energy, B store in pinned host memory (out of core) or on the
+    device.  --canonical o,v,naux[,occ_block[,host|device]]; nao = o + v; the packed integrals are generated and fed in aux
+    blocks (never resident at once).  Reports the device time of the two phases (CUDA events) and the panel traffic."""
+    import torch
+
+    import paper_2412_18553_b200 as sie
+
+    torch.cuda.set_device(0)
+    f = args.canonical.split(",")
+    o, v, naux = int(f[0]), int(f[1]), int(f[2])
+    occ_block = int(f[3]) if len(f) > 3 else 0
+    store = f[4] if len(f) > 4 else "host"
+    spec = ClusterSpec(10, 0, o + v, o, v, naux, 0)
+    x = make_cluster(spec)
+    cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()  # noqa: E731
+    s = sie.CanonicalSolver(spec.nao, o, v, naux, occ_block=occ_block, store=store)
+    info = s.info()
+    blk = max(8, min(naux, int(args.stream_gb * 1e9) // (8 * spec.npair)) // 8 * 8)
+    pinned = torch.empty((blk, spec.npair), dtype=torch.float64, pin_memory=True)
+    Ld = torch.empty((blk, spec.npair), dtype=torch.float64, device="cuda")
+    C_occ, C_vir, e_occ, e_vir = cu(x.C_occ), cu(x.C_vir), cu(x.e_occ), cu(x.e_vir)
+    ncpu = max(1, min(32, os.cpu_count() or 8))
+    l0 = sie.launch_count()
+    t_tr = 0.0
+    with ClockSampler(0) as cs:
+        for p0 in range(0, naux, blk):
+            p1 = min(naux, p0 + blk)
+            x.L_block(p0, p1, out=pinned.numpy()[: p1 - p0], threads=ncpu)
+            Ld[: p1 - p0].copy_(pinned[: p1 - p0])
+            torch.cuda.synchronize()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record()
+            s.transform(C_occ, C_vir, Ld[: p1 - p0], p0, p1)
+            ev1.record()
+            torch.cuda.synchronize()
+            t_tr += ev0.elapsed_time(ev1)
+        E = s.energy(e_occ, e_vir)  # warm-up pass (same work)
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        E = s.energy(e_occ, e_vir)
+        ev1.record()
+        torch.cuda.synchronize()
+        t_en = ev0.elapsed_time(ev1)
+    peak = max(max(sie.sie_dfmp2_probe_fp64(k, 40000, 2)[0] for _ in range(3)) for k in (0, 1))
+    fl = alg_flops(spec)
+    f_pair = 1.0 * o * (o + 1) * v * v * naux  # unordered occupied pairs, full v x v block each: the minimum
+    nb = info["n_occ_blocks"]
+    panel_bytes = (nb + nb * (nb - 1) // 2) * 8.0 * info["occ_block"] * v * ((naux + 7) // 8 * 8)
+    line = {"mode": "canonical (NEXT-2)", "nocc": o, "nvir": v, "nao": o + v, "naux": naux, "store": store, "info": info,
+            "E_MP2": float(E.cpu()[0]), "transform_ms": t_tr, "transform_tflops": (fl["A1"] + fl["A2"]) / (t_tr * 1e-3) * 1e-12,
+            "energy_ms": t_en, "energy_tflops": f_pair / (t_en * 1e-3) * 1e-12, "energy_frac_of_fp64_peak": f_pair / (t_en * 1e-3) * 1e-12 / peak,
+            "fp64_peak_probe": peak, "panel_bytes_to_device_per_energy": panel_bytes,
+            "panel_gbs": panel_bytes / (t_en * 1e-3) * 1e-9, "b_store_bytes": s.bstore_bytes, "workspace_bytes": s.workspace_bytes,
+            "gpu_launches": sie.launch_count() - l0, "clocks": cs.summary(),
+            "note": "device time of each phase (CUDA events); packed integrals generated and fed in aux blocks; data synthetic"}
+    print(json.dumps(line))
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -688,8 +748,12 @@ def main() -> None:
     ap.add_argument("--streamed", action="store_true", help="feed the packed integrals in aux blocks generated on the fly "
                                                              "(sweep points that do not fit in HBM; not a bench line)")
     ap.add_argument("--stream-gb", type=float, default=8.0, help="size of one streamed aux block in GB")
+    ap.add_argument("--canonical", default="", help="o,v,naux[,occ_block[,host|device]]: whole-system canonical DF-MP2 energy "
+                                                     "(NEXT-2, out of core; not a bench line)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.canonical:
+        run_canonical(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.streamed:
         run_streamed(args)
