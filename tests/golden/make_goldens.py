@@ -11,6 +11,8 @@ Cases (BASELINE.json configs; generator recipe in workloads/gen.py):
   config3_v256   config 3 with C_vir zeroed outside workloads.virtual_subset(spec, 256): the oracle runs the
                  compressed problem (same bytes for the 256 kept columns), G, E, and gamma_occ (Eq. S18)
   config4_k      sweep point k (o=64, v=256/512/1024/2048): G, E_frag (rank 32), E(P=I); gamma_occ for k <= 1
+  config4_3_v256 the v=2048 point (nao=2112, naux=8448, packed integrals 150.8 GB) with C_vir zeroed outside 256 seeded
+                 columns: the compressed problem for the oracle, the full-size streamed launch for the GPU; G, E, gamma_occ
 
 What is computed is exactly oracle.transform_block (O1-O3), oracle.pair_G (O4-O6) and oracle.trace (O7) as they
 stand.  The only thing this script adds is bookkeeping: the aux index is fed in blocks (the oracle's own p0/p1
@@ -171,6 +173,8 @@ def main():
             single(case, config_specs(3)[0], a.cache, a.threads, a.jchunk)
         elif case == "config3_v256":
             single(case, config_specs(3)[0], a.cache, a.threads, a.jchunk, subset=256, want_gamma=True)
+        elif case == "config4_3_v256":
+            single(case, config_specs(4)[6], a.cache, a.threads, a.jchunk, subset=256, want_gamma=True)
         elif case.startswith("config4_"):
             k = int(case.split("_")[1])
             single(case, config_specs(4)[2 * k], a.cache, a.threads, a.jchunk, want_gamma=(k <= 1))

@@ -146,11 +146,21 @@ def test_config3_dense_aux_256_dense_virtuals_matches_golden(config3_inputs):
 
 
 # ---------------------------------------------------------------------------------------------- config 4: the size sweep
-@pytest.mark.parametrize("k", [0, 1, 2, 3])
+@pytest.mark.parametrize("k", [0, 1, 2, 3, "3_v256"])
 def test_config4_sweep_point_matches_golden(k):
+    """k = "3_v256": the v = 2048 point with C_vir zeroed outside 256 seeded columns (dense aux, dense occupied): the GPU
+    streams all 150.8 GB of packed integrals and runs the full-size launch, the oracle ran the compressed problem."""
     meta, arr = _golden(f"config4_{k}")
+    sub = isinstance(k, str)
+    k = 3 if sub else k
     spec = config_specs(4)[2 * k]  # rank-32 projector; the P = I run shares G (A-15)
     x = make_cluster(spec)
+    if sub:
+        virt = virtual_subset(spec, 256)
+        assert np.array_equal(virt, arr["virtual_subset"])
+        Cz = np.zeros_like(x.C_vir)
+        Cz[:, virt] = x.C_vir[:, virt]
+        x.C_vir = Cz
     _need_gb(8 * spec.naux * spec.npair / 2**30 + 16 if k < 3 else 40)
     s = sie.ClusterSolver(spec.nao, spec.nocc, spec.nvir, spec.naux)
     C_occ, C_vir = _cu(x.C_occ), _cu(x.C_vir)
