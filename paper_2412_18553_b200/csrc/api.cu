@@ -679,7 +679,8 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
         {
             ProfSpan ps(p.prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc),
-                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8, mode, st));
+                                reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8,
+                                (mode == 0 && o <= 64) ? 3 : mode, st));
         }
         rc.gpart = gpart;
         rc.o8 = p.o8;
@@ -1113,8 +1114,10 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_CUDA(cudaMemcpyAsync(ws + off_tiles, tiles.data(), tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
             SIE_CUDA(cudaMemsetAsync(ws + off_tiles + tiles.size() * sizeof(PairTile), 0, 256, st));
             ProfSpan ps(prof, ST_PAIR, st);
+            bool any_small = false;
+            for (int k : order) any_small = any_small || plans[k].o <= 64;
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
-                                (int)tiles.size(), ncta, tmax, mode, st));
+                                (int)tiles.size(), ncta, tmax, (mode == 0 && any_small) ? 3 : mode, st));
         }
         // clusters with nocc > 128: the any-size slab/Gram route, one cluster at a time on shared scratch
         for (int k = 0; k < ncluster; ++k) {

@@ -68,7 +68,8 @@ struct PairGeom {                  // tile configuration facts for host-side pla
 };
 PairGeom pair_geom();
 size_t pair_smem_bytes();
-// mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma), 2 energy only with a low-rank projector; one mode per launch
+// mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma), 2 energy only with a low-rank projector, 3 = mode 0 through the
+// instantiation whose strips for o <= 64 are epilogue_strip_small (same sums; chosen by the caller when such clusters exist); one mode per launch
 int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, int mode, cudaStream_t st);
 
 struct ReduceCluster {             // per cluster, device array
