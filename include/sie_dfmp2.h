@@ -58,7 +58,11 @@ enum {
     SIE_FLAG_PROFILE = 8u,   /* bracket every launch group with CUDA events; read with *_timing (below) */
     SIE_FLAG_RDM_OCC = 16u,  /* sie_dfmp2_batch only: compute the occupied 1-RDM block of every cluster instead of the
                                 energy (3b): G_out receives gamma, E_out receives Tr gamma, P_frag is ignored */
-    SIE_FLAG_RDM_VIR = 32u   /* sie_dfmp2_plan only: reserve the workspace sie_dfmp2_rdm_vir (3c) needs (three amplitude slabs) */
+    SIE_FLAG_RDM_VIR = 32u,  /* sie_dfmp2_plan only: reserve the workspace sie_dfmp2_rdm_vir (3c) needs (three amplitude slabs) */
+    SIE_FLAG_STAGE_FULL = 64u /* sie_dfmp2_plan with SIE_FLAG_HOST_IO: stage the WHOLE packed tensor in the workspace (naux * npair
+                                 doubles more) instead of a two-buffer ring.  The upload of a cluster then never waits for its own
+                                 GEMMs, so with two plans on two streams the integrals of cluster n+1 travel while the pair stage of
+                                 cluster n runs (transform of n+1 enqueued before energy of n) */
 };
 
 /*

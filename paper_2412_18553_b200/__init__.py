@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     SIE_FLAG_RDM_OCC,
     SIE_FLAG_RDM_VIR,
     SIE_FLAG_REFERENCE,
+    SIE_FLAG_STAGE_FULL,
     SIE_FLAG_VALIDATE,
     CanonicalSolver,
     ClusterSolver,

@@ -13,7 +13,7 @@ from typing import List, Optional, Sequence, Tuple
 import torch
 
 SIE_OK, SIE_EINVAL, SIE_ENOMEM, SIE_ECUDA, SIE_ESTATE, SIE_EGAP, SIE_EUNSUPPORTED = range(7)
-SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO, SIE_FLAG_PROFILE, SIE_FLAG_RDM_OCC, SIE_FLAG_RDM_VIR = 1, 2, 4, 8, 16, 32
+SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO, SIE_FLAG_PROFILE, SIE_FLAG_RDM_OCC, SIE_FLAG_RDM_VIR, SIE_FLAG_STAGE_FULL = 1, 2, 4, 8, 16, 32, 64
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsie_dfmp2.so")

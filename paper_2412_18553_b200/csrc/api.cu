@@ -213,12 +213,15 @@ struct sie_dfmp2_plan_s {
     std::vector<std::pair<int, int>> covered;
     long long covered_rows = 0;
     const void* c_ready_ws = nullptr;  // workspace for which the transposed coefficient copies are valid
+    const void* tiles_ws = nullptr;    // workspace that holds the (static) tile list
     const double* dC_occ = nullptr;    // device pointers of the coefficients used by the transform
     const double* dC_vir = nullptr;
     // HOST_IO copy pipeline
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr}, ev_fork = nullptr;
     int stage_turn = 0;
+    bool stage_full = false;
+    std::vector<cudaEvent_t> ev_chunk;  // SIE_FLAG_STAGE_FULL: one "chunk landed" event per staged chunk of a call
 };
 
 namespace {
@@ -250,7 +253,9 @@ enum { CARVE_NONE = 0, CARVE_MEMBER = 1, CARVE_ALL = 2 };  // what plan_init lay
 int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int aux_block, unsigned flags, int carve) {
     if (nao < 1 || nocc < 1 || nvir < 1 || naux < 1 || aux_block < 0) return SIE_EINVAL;
     if ((long long)nocc + nvir > nao) return SIE_EINVAL;
-    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_VIR)) return SIE_EINVAL;
+    if (flags & ~(SIE_FLAG_VALIDATE | SIE_FLAG_REFERENCE | SIE_FLAG_HOST_IO | SIE_FLAG_PROFILE | SIE_FLAG_RDM_VIR | SIE_FLAG_STAGE_FULL))
+        return SIE_EINVAL;
+    if ((flags & SIE_FLAG_STAGE_FULL) && !(flags & SIE_FLAG_HOST_IO)) return SIE_EINVAL;
     p.nao = nao;
     p.o = nocc;
     p.v = nvir;
@@ -332,7 +337,10 @@ int plan_init(sie_dfmp2_plan_s& p, int nao, int nocc, int nvir, int naux, int au
         p.off_rc = c.take(sizeof(ReduceCluster));
         if (flags & SIE_FLAG_HOST_IO) {
             p.stage_buf_bytes = align_up((size_t)p.cblk * p.npair * 8, 256);
-            p.off_stage = c.take(2 * p.stage_buf_bytes);
+            p.stage_full = (flags & SIE_FLAG_STAGE_FULL) && !p.ref;
+            // two-buffer ring, or (SIE_FLAG_STAGE_FULL) room for the whole packed tensor so that the upload of a cluster never
+            // waits for the GEMMs of an earlier chunk and can run under the pair stage of ANOTHER plan on another stream
+            p.off_stage = c.take(p.stage_full ? align_up((size_t)naux * p.npair * 8, 256) : 2 * p.stage_buf_bytes);
             size_t d = 0;
             p.io_Cocc = d, d += (size_t)nao * nocc;
             p.io_Cvir = d, d += (size_t)nao * nvir;
@@ -467,7 +475,21 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
             const int c1 = std::min(q1, c0 + step), np = c1 - c0;
             const double* Lq = L + (size_t)(c0 - p0) * p.npair;
             int buf = 0;
-            if (host_L) {
+            if (host_L && p.stage_full) {
+                // whole-tensor staging: chunk [c0,c1) has its own place, nothing to wait for but the fork of this call
+                sie_dfmp2_plan_s& po = pipe_owner;
+                const size_t ci = (size_t)used;
+                while (po.ev_chunk.size() <= ci) {
+                    cudaEvent_t e;
+                    SIE_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                    po.ev_chunk.push_back(e);
+                }
+                unsigned char* dst = sc.stage + (size_t)c0 * p.npair * 8;
+                SIE_CUDA(cudaMemcpyAsync(dst, Lq, (size_t)np * p.npair * 8, cudaMemcpyHostToDevice, po.copy_stream));
+                SIE_CUDA(cudaEventRecord(po.ev_chunk[ci], po.copy_stream));
+                SIE_CUDA(cudaStreamWaitEvent(st, po.ev_chunk[ci], 0));
+                Lq = reinterpret_cast<const double*>(dst);
+            } else if (host_L) {
                 sie_dfmp2_plan_s& po = pipe_owner;
                 buf = po.stage_turn++ & 1;
                 unsigned char* dst = sc.stage + (size_t)buf * sc.stage_buf_bytes;
@@ -480,7 +502,7 @@ int transform_rows(sie_dfmp2_plan_s& p, sie_dfmp2_plan_s& pipe_owner, Prof& prof
             if (used >= p.max_jobs) return SIE_EINVAL;  // cannot happen: max_jobs counts every chunk and sub-block
             SIE_TRY(make_a1_job(jobs[0], p, sc.CoT, Lq, np, sc.H, c0 - q0, pb));
             SIE_TRY(launch_jobs(jobs, true, arena + (size_t)used++ * sizeof(XJob), p.num_sms, prof, ST_T1, st));
-            if (host_L) SIE_CUDA(cudaEventRecord(pipe_owner.ev_consumed[buf], st));
+            if (host_L && !p.stage_full) SIE_CUDA(cudaEventRecord(pipe_owner.ev_consumed[buf], st));
         }
         if (used >= p.max_jobs) return SIE_EINVAL;
         SIE_TRY(make_a2_job(jobs[0], p, sc.CvT, sc.H, pb, Bmat, q0));
@@ -516,6 +538,26 @@ int fill_pair_cluster(const sie_dfmp2_plan_s& p, const double* Bmat, const doubl
     d.kp = kp;
     d.t8 = p.t8;
     d.tx_bytes = 2u * 8u * (uint32_t)p.t8 * 8u;
+    return SIE_OK;
+}
+
+// HOST_IO upload of a small operand.  Pinned (host-registered) memory is read by a copy kernel through its mapped device
+// address, so the upload does not queue on the host-to-device copy engine behind a large staging copy of another plan;
+// pageable memory takes cudaMemcpyAsync.
+int stage_small(double* dst, const double* src, size_t n, cudaStream_t st) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, src) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+        return launch_copy_f64(static_cast<const double*>(at.devicePointer), dst, n, st);
+    (void)cudaGetLastError();
+    SIE_CUDA(cudaMemcpyAsync(dst, src, n * 8, cudaMemcpyHostToDevice, st));
+    return SIE_OK;
+}
+
+// the static tile list of a fused plan goes to the workspace once per workspace (first transform), not with every energy call
+int upload_tiles(sie_dfmp2_plan_s& p, unsigned char* ws, cudaStream_t st) {
+    if (!p.fused || p.tiles_ws == ws) return SIE_OK;
+    SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+    p.tiles_ws = ws;
     return SIE_OK;
 }
 
@@ -592,6 +634,7 @@ int sie_dfmp2_transform(sie_dfmp2_plan_t plan, void* workspace, const double* C_
             dCv = io + p.io_Cvir;
         }
         SIE_TRY(prepare_coeffs(p, p.prof, sc, dCo, dCv, st));
+        SIE_TRY(upload_tiles(p, ws, st));
         p.dC_occ = dCo;
         p.dC_vir = dCv;
         p.c_ready_ws = workspace;
@@ -619,12 +662,12 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
     double* io = reinterpret_cast<double*>(ws + p.off_io);
     if (host) {
         if (p.flags & SIE_FLAG_VALIDATE) SIE_TRY(check_gap_host(e_occ, e_vir, o, v));
-        SIE_CUDA(cudaMemcpyAsync(io + p.io_eo, e_occ, (size_t)o * 8, cudaMemcpyHostToDevice, st));
-        SIE_CUDA(cudaMemcpyAsync(io + p.io_ev, e_vir, (size_t)v * 8, cudaMemcpyHostToDevice, st));
+        SIE_TRY(stage_small(io + p.io_eo, e_occ, (size_t)o, st));
+        SIE_TRY(stage_small(io + p.io_ev, e_vir, (size_t)v, st));
         de_occ = io + p.io_eo;
         de_vir = io + p.io_ev;
         if (P_frag) {
-            SIE_CUDA(cudaMemcpyAsync(io + p.io_P, P_frag, (size_t)o * o * 8, cudaMemcpyHostToDevice, st));
+            SIE_TRY(stage_small(io + p.io_P, P_frag, (size_t)o * o, st));
             dP = io + p.io_P;
         }
         dE = io + p.io_E;
@@ -672,8 +715,8 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
         SIE_TRY(fill_pair_cluster(p, Bmat, de_occ, de_vir, gpart, p.kp, pc));
         pc.gate = 1;  // one cluster: all tiles cost the same, keep the CTAs in K-lockstep for L2
         pc.mode = mode;
-        SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
-        SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+        SIE_TRY(launch_poke(&pc, sizeof pc, ws + p.off_desc, st));
+        SIE_TRY(upload_tiles(p, ws, st));
         SIE_CUDA(cudaMemsetAsync(ws + p.off_tiles + p.tiles.size() * sizeof(PairTile), 0, 256, st));
         SIE_CUDA(cudaMemsetAsync(gpart, 0, (size_t)p.ncta * p.kp * p.o8 * p.o8 * 8, st));
         {
@@ -686,7 +729,7 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
         rc.o8 = p.o8;
         rc.nslots = p.ncta * p.kp;
     }
-    SIE_CUDA(cudaMemcpyAsync(ws + p.off_rc, &rc, sizeof rc, cudaMemcpyHostToDevice, st));
+    SIE_TRY(launch_poke(&rc, sizeof rc, ws + p.off_rc, st));
     {
         ProfSpan ps(p.prof, ST_REDUCE, st);
         SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
@@ -726,9 +769,9 @@ int sie_dfmp2_energy_lowrank(sie_dfmp2_plan_t plan, void* workspace, const doubl
     double* io = reinterpret_cast<double*>(ws + p.off_io);
     if (host) {
         if (p.flags & SIE_FLAG_VALIDATE) SIE_TRY(check_gap_host(e_occ, e_vir, o, v));
-        SIE_CUDA(cudaMemcpyAsync(io + p.io_eo, e_occ, (size_t)o * 8, cudaMemcpyHostToDevice, st));
-        SIE_CUDA(cudaMemcpyAsync(io + p.io_ev, e_vir, (size_t)v * 8, cudaMemcpyHostToDevice, st));
-        SIE_CUDA(cudaMemcpyAsync(io + p.io_P, Q, (size_t)o * r * 8, cudaMemcpyHostToDevice, st));  // r <= o: fits the P slot
+        SIE_TRY(stage_small(io + p.io_eo, e_occ, (size_t)o, st));
+        SIE_TRY(stage_small(io + p.io_ev, e_vir, (size_t)v, st));
+        SIE_TRY(stage_small(io + p.io_P, Q, (size_t)o * r, st));  // r <= o: fits the P slot
         de_occ = io + p.io_eo;
         de_vir = io + p.io_ev;
         dQ = io + p.io_P;
@@ -770,15 +813,15 @@ int sie_dfmp2_energy_lowrank(sie_dfmp2_plan_t plan, void* workspace, const doubl
         rc.nslots = p.ncta * p.kp;
     }
     rc.gpart = gpart;
-    SIE_CUDA(cudaMemcpyAsync(ws + p.off_desc, &pc, sizeof pc, cudaMemcpyHostToDevice, st));
-    SIE_CUDA(cudaMemcpyAsync(ws + p.off_tiles, p.tiles.data(), p.tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
+    SIE_TRY(launch_poke(&pc, sizeof pc, ws + p.off_desc, st));
+    SIE_TRY(upload_tiles(p, ws, st));
     SIE_CUDA(cudaMemsetAsync(ws + p.off_tiles + p.tiles.size() * sizeof(PairTile), 0, 256, st));
     {
         ProfSpan ps(p.prof, ST_PAIR, st);
         SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc), reinterpret_cast<const PairTile*>(ws + p.off_tiles),
                             (int)p.tiles.size(), p.ncta, p.t8, pc.mode, st));
     }
-    SIE_CUDA(cudaMemcpyAsync(ws + p.off_rc, &rc, sizeof rc, cudaMemcpyHostToDevice, st));
+    SIE_TRY(launch_poke(&rc, sizeof rc, ws + p.off_rc, st));
     {
         ProfSpan ps(p.prof, ST_REDUCE, st);
         SIE_TRY(launch_reduce(reinterpret_cast<const ReduceCluster*>(ws + p.off_rc), 1, st));
@@ -1187,6 +1230,7 @@ int sie_dfmp2_destroy(sie_dfmp2_plan_t plan) {
             cudaEventDestroy(plan->ev_consumed[i]);
         }
         cudaEventDestroy(plan->ev_fork);
+        for (cudaEvent_t e : plan->ev_chunk) cudaEventDestroy(e);
         cudaStreamDestroy(plan->copy_stream);
     }
     delete plan;

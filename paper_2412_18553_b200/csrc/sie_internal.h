@@ -43,6 +43,10 @@ struct TJob {
 };
 int launch_transpose_jobs(const TJob* d_jobs, int njobs, int max_rows, int max_cols, cudaStream_t st);
 
+// descriptor / small-operand writers that do not use the host-to-device copy engine (see transform.cu)
+int launch_poke(const void* payload, size_t nbytes, void* dst, cudaStream_t st);      // nbytes <= 512, multiple of 8
+int launch_copy_f64(const double* src, double* dst, size_t n, cudaStream_t st);       // src device or mapped pinned host
+
 // ---- pair.cu -----------------------------------------------------------------------------------
 struct alignas(128) PairCluster {  // one per cluster, lives in the workspace (global memory)
     CUtensorMap map;               // B as the plain matrix {naux, nocc*nvir, 1}, box {8, t8, 1}

@@ -7,6 +7,9 @@
 // C = A * Bop^T over K-major operands, used for both half transforms of every cluster of a call in one launch per
 // stage: A1 gathers its Bop operand straight from the packed triangle (no unpacked square in HBM), A2 lands B directly
 // in its final [a][i][P] layout through an output-column remap.
+#include <algorithm>
+#include <cstring>
+
 #include "mma_pipeline.cuh"
 #include "sie_internal.h"
 #include "../../include/sie_dfmp2.h"
@@ -277,6 +280,43 @@ int launch_transpose_jobs(const TJob* d_jobs, int njobs, int max_rows, int max_c
         transpose_jobs_kernel<<<grid, block, 0, st>>>(d_jobs + z0);
         note_launch();
     }
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SIE_OK : set_cuda_error(e);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Small device-side writers that keep descriptor and operand uploads OFF the host-to-device copy engine: that engine
+// serves copies in order, so a 256-byte descriptor enqueued behind the 27.7 GB integral upload of the NEXT cluster
+// (another plan, another stream) would hold this cluster's pair stage back for half a second.
+struct PokeArgs {
+    unsigned long long payload[64];  // up to 512 bytes, travels as a kernel parameter
+    void* dst;
+    int nwords;
+};
+__global__ void poke_kernel(const PokeArgs a) {
+    unsigned long long* d = static_cast<unsigned long long*>(a.dst);
+    for (int i = threadIdx.x; i < a.nwords; i += blockDim.x) d[i] = a.payload[i];
+}
+int launch_poke(const void* payload, size_t nbytes, void* dst, cudaStream_t st) {
+    if (nbytes > 512 || (nbytes & 7)) return SIE_EINVAL;
+    PokeArgs a;
+    std::memcpy(a.payload, payload, nbytes);
+    a.dst = dst;
+    a.nwords = (int)(nbytes / 8);
+    poke_kernel<<<1, 64, 0, st>>>(a);
+    note_launch();
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SIE_OK : set_cuda_error(e);
+}
+// dst[i] = src[i]; src may be pinned host memory mapped into the device address space (read over PCIe by the SMs)
+__global__ void copy_f64_kernel(const double* __restrict__ src, double* __restrict__ dst, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) dst[i] = src[i];
+}
+int launch_copy_f64(const double* src, double* dst, size_t n, cudaStream_t st) {
+    if (n == 0) return SIE_OK;
+    const int grid = (int)std::min<size_t>(64, (n + 255) / 256);
+    copy_f64_kernel<<<grid, 256, 0, st>>>(src, dst, n);
+    note_launch();
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SIE_OK : set_cuda_error(e);
 }

@@ -242,3 +242,24 @@ def test_launch_counter_counts_our_kernels():
     spec = config_specs(0, "std")[0]
     gpu_run(spec)
     assert sie.launch_count() - before >= 5  # coefficient transposes, A1, A2, pair, reduce
+
+
+def test_host_io_whole_tensor_staging_and_two_plans_on_two_streams():
+    """SIE_FLAG_STAGE_FULL: the packed tensor is staged whole; two plans on two streams, the transform of the second
+    enqueued before the energy of the first (the software pipeline of bench.py's e2e arm) give the device-path results."""
+    specs = [ClusterSpec(60, k, 70, 10, 60, 90, 3, "std") for k in range(2)]
+    xs = [make_cluster(s) for s in specs]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
+    fl = binding.SIE_FLAG_HOST_IO | binding.SIE_FLAG_STAGE_FULL
+    solvers = [sie.ClusterSolver(s.nao, s.nocc, s.nvir, s.naux, aux_block=32, flags=fl) for s in specs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    hs = [dict(C_occ=pin(x.C_occ), C_vir=pin(x.C_vir), L=pin(x.L_packed()), e_occ=pin(x.e_occ), e_vir=pin(x.e_vir), P=pin(x.P_frag)) for x in xs]
+    solvers[0].transform(hs[0]["C_occ"], hs[0]["C_vir"], hs[0]["L"], 0, specs[0].naux, stream=streams[0])
+    solvers[1].transform(hs[1]["C_occ"], hs[1]["C_vir"], hs[1]["L"], 0, specs[1].naux, stream=streams[1])
+    out = [solvers[k].energy(hs[k]["e_occ"], hs[k]["e_vir"], hs[k]["P"], stream=streams[k]) for k in range(2)]
+    torch.cuda.synchronize()
+    for k in range(2):
+        check(specs[k], float(out[k][0][0]), out[k][1].numpy())
+        solvers[k].close()
+    with pytest.raises(sie.SieError):  # the flag needs SIE_FLAG_HOST_IO
+        sie.sie_dfmp2_plan(70, 10, 60, 90, 0, binding.SIE_FLAG_STAGE_FULL)
