@@ -48,14 +48,35 @@ __global__ void slab_combine_kernel(const double* __restrict__ V, int o, int v, 
     }
 }
 
+// V[r][c] = V[c][r] for r > c (square n x n, leading dimension ld): completes a matrix whose upper triangle was computed
+__global__ void mirror_lower_kernel(double* __restrict__ V, long long n, long long ld) {
+    __shared__ double tile[32][33];
+    const long long bc = blockIdx.x, br = blockIdx.y;  // destination tile (rows br, columns bc), only br >= bc
+    if (br < bc) return;
+    for (int rr = threadIdx.y; rr < 32; rr += 8) {  // read the source tile (rows bc-block, columns br-block), coalesced
+        const long long r = bc * 32 + rr, c = br * 32 + threadIdx.x;
+        tile[rr][threadIdx.x] = (r < n && c < n) ? V[r * ld + c] : 0.0;
+    }
+    __syncthreads();
+    for (int rr = threadIdx.y; rr < 32; rr += 8) {
+        const long long r = br * 32 + rr, c = bc * 32 + threadIdx.x;
+        if (r < n && c < n && r > c) V[r * ld + c] = tile[threadIdx.x][rr];
+    }
+}
+
 GeneralGeom general_geom(int o, int v, int num_sms) {
     GeneralGeom g{};
     int Kb = 1;
     while (Kb * 2 <= std::min(o, 128) && (double)v * o * v * (Kb * 2) * 8.0 <= (double)((size_t)1 << 30)) Kb *= 2;
+    // When the whole integral matrix M[(a,i)][(b,k)] = (ia|kb) fits (<= 8 GB: the large-occ x small-vir sub-space of the BNO
+    // step, and every small cluster), ONE occupied block covers everything and the slab GEMM becomes a SYRK: only the tile
+    // rows' upper parts are computed and the lower triangle is mirrored — the o^2 v^2 naux minimum instead of twice that.
+    g.full = (double)v * o * (double)v * o * 8.0 <= 8.0 * (double)((size_t)1 << 30);
+    if (g.full) Kb = o;
     g.Kb = Kb;
     g.ldc = (int)align_up((size_t)v * Kb, 8);
     g.slab_bytes = align_up((size_t)v * o * g.ldc * 8, 256);
-    g.ok = (double)g.slab_bytes <= (double)((size_t)4 << 30);
+    g.ok = (double)g.slab_bytes <= (double)((size_t)(g.full ? 9 : 4) << 30);
     for (int which = 0; which < 2; ++which) {  // Gram of the occupied (0) / virtual (1) block: split K until ~4 waves of tiles
         const int n = which ? v : o;
         const int mt = (n + 127) / 128, tiles = mt * ((n + 127) / 128);
@@ -65,6 +86,7 @@ GeneralGeom general_geom(int o, int v, int num_sms) {
     }
     g.slots_bytes = align_up(std::max((size_t)g.nsplit_occ * o * o, (size_t)g.nsplit_vir * v * v) * 8, 256);
     g.max_jobs = 1 + std::max(g.nsplit_occ, g.nsplit_vir);
+    if (g.full) g.max_jobs += (int)(((long long)v * o + 127) / 128);  // one SYRK job per 128-row block
     return g;
 }
 
@@ -86,6 +108,50 @@ int general_pair(const GeneralGeom& g, const double* Bmat, int o, int v, int nau
         const int k0 = blk * g.Kb;
         unsigned char* d_jobs = arena + (size_t)blk * g.max_jobs * sizeof(XJob);
         // ---- 1. slab GEMM
+        int first_gram_job = 1;
+        if (g.full) {
+            // SYRK of the (v*o) x naux matrix B: one job per 128-row block r, columns from r*128 on; then mirror
+            jobs.clear();
+            const int nrb = (int)((rows + 127) / 128);
+            long long t = 0;
+            for (int r = 0; r < nrb; ++r) {
+                const long long r0 = (long long)r * 128, M = std::min<long long>(128, rows - r0), N = rows - r0;
+                XJob J;
+                std::memset(&J, 0, sizeof J);
+                const double* Br = Bmat + r0 * naux_ld;
+                int rc = make_tensor_map_3d(&J.mapA, Br, naux, M, 1, (uint64_t)naux_ld * 8, (uint64_t)M * naux_ld * 8, 8, (uint32_t)(8 * ((M + 7) / 8)), 1);
+                if (rc != SIE_OK) return rc;
+                rc = make_tensor_map_3d(&J.mapB, Br, naux, N, 1, (uint64_t)naux_ld * 8, (uint64_t)N * naux_ld * 8, 8, 128, 1);
+                if (rc != SIE_OK) return rc;
+                J.n_total = N;
+                J.M = (int)M;
+                J.m8 = (int)((M + 7) / 8);
+                J.m_tiles = 1;
+                J.n_tiles = (int)((N + 127) / 128);
+                J.kblocks = (naux + 7) / 8;
+                J.b_c1_mul = 128;
+                J.out.base = V + r0 * g.ldc + r0;
+                J.out.ld_m = g.ldc;
+                J.out.M = (int)M;
+                J.out.inner = g.ldc;
+                J.out.valid_inner = (int)N;
+                J.out.stride_outer = 0;
+                J.out.n_lin_total = N;
+                J.tile_begin = (int)t;
+                t += J.n_tiles;
+                jobs.push_back(J);
+            }
+            ce = cudaMemcpyAsync(d_jobs, jobs.data(), jobs.size() * sizeof(XJob), cudaMemcpyHostToDevice, st);
+            if (ce != cudaSuccess) return set_cuda_error(ce);
+            int rc = launch_xform_gemm(false, reinterpret_cast<const XJob*>(d_jobs), (int)jobs.size(), (int)t, num_sms, st);
+            if (rc != SIE_OK) return rc;
+            const unsigned nb32 = (unsigned)((rows + 31) / 32);
+            mirror_lower_kernel<<<dim3(nb32, nb32), dim3(32, 8), 0, st>>>(V, rows, g.ldc);
+            note_launch();
+            ce = cudaGetLastError();
+            if (ce != cudaSuccess) return set_cuda_error(ce);
+            first_gram_job = (int)jobs.size();
+        } else {
         XJob J;
         std::memset(&J, 0, sizeof J);
         int rc = make_tensor_map_3d(&J.mapA, Bmat, naux, rows, 1, (uint64_t)naux_ld * 8, (uint64_t)rows * naux_ld * 8, 8, 128, 1);
@@ -113,6 +179,7 @@ int general_pair(const GeneralGeom& g, const double* Bmat, int o, int v, int nau
         if (ce != cudaSuccess) return set_cuda_error(ce);
         rc = launch_xform_gemm(false, reinterpret_cast<const XJob*>(d_jobs), 1, J.m_tiles * J.n_tiles, num_sms, st);
         if (rc != SIE_OK) return rc;
+        }
         // ---- 2. amplitudes and the 2x - x~ combination
         slab_combine_kernel<<<num_sms * 8, 256, 0, st>>>(V, o, v, g.Kb, k0, g.ldc, e_occ, e_vir, mode, S1, S2);
         note_launch();
@@ -131,7 +198,7 @@ int general_pair(const GeneralGeom& g, const double* Bmat, int o, int v, int nau
             XJob Q;
             std::memset(&Q, 0, sizeof Q);
             const int mt = (n + 127) / 128, m8 = ((n + mt - 1) / mt + 7) / 8;
-            rc = make_tensor_map_3d(&Q.mapA, S1, (uint64_t)Ktot, n, 1, (uint64_t)Ktot * 8, (uint64_t)Ktot * 8 * n, 8, 8 * m8, 1);
+            int rc = make_tensor_map_3d(&Q.mapA, S1, (uint64_t)Ktot, n, 1, (uint64_t)Ktot * 8, (uint64_t)Ktot * 8 * n, 8, 8 * m8, 1);
             if (rc != SIE_OK) return rc;
             rc = make_tensor_map_3d(&Q.mapB, S2, (uint64_t)Ktot, n, 1, (uint64_t)Ktot * 8, (uint64_t)Ktot * 8 * n, 8, 128, 1);
             if (rc != SIE_OK) return rc;
@@ -155,9 +222,10 @@ int general_pair(const GeneralGeom& g, const double* Bmat, int o, int v, int nau
             t += Q.m_tiles * Q.n_tiles;
             jobs.push_back(Q);
         }
-        ce = cudaMemcpyAsync(d_jobs + sizeof(XJob), jobs.data(), jobs.size() * sizeof(XJob), cudaMemcpyHostToDevice, st);
+        ce = cudaMemcpyAsync(d_jobs + (size_t)first_gram_job * sizeof(XJob), jobs.data(), jobs.size() * sizeof(XJob), cudaMemcpyHostToDevice, st);
         if (ce != cudaSuccess) return set_cuda_error(ce);
-        rc = launch_xform_gemm(false, reinterpret_cast<const XJob*>(d_jobs + sizeof(XJob)), (int)jobs.size(), t, num_sms, st);
+        int rc = launch_xform_gemm(false, reinterpret_cast<const XJob*>(d_jobs + (size_t)first_gram_job * sizeof(XJob)), (int)jobs.size(), t,
+                                   num_sms, st);
         if (rc != SIE_OK) return rc;
     }
     *nslots = nsplit;

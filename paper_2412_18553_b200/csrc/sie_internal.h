@@ -96,6 +96,7 @@ struct GeneralGeom {
     int nsplit_occ, nsplit_vir;  // K splits (= partial slots) of the Gram GEMM of the occupied / virtual block
     int max_jobs;                // job descriptors per occupied block
     bool ok;                     // false: one slab would exceed 4 GB (sizes beyond this route)
+    bool full;                   // one occupied block covers the cluster: the slab GEMM is a SYRK (upper tiles + mirror)
     size_t slab_bytes, slots_bytes;
 };
 GeneralGeom general_geom(int o, int v, int num_sms);

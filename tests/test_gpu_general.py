@@ -252,3 +252,19 @@ def test_canonical_call_order():
         s.energy(torch.zeros(4, dtype=torch.float64, device="cuda"), torch.ones(16, dtype=torch.float64, device="cuda"))
     assert ei.value.status == binding.SIE_ESTATE
     s.close()
+
+
+def test_general_route_block_slab_mode_large_integral_matrix():
+    """(o, v) = (129, 260): the integral matrix (o v)^2 doubles is 9 GB, above the whole-matrix SYRK limit, so the general
+    route runs its block-slab mode (power-of-two occupied blocks, 3-D tensor map for the column operand, ragged last
+    block).  E, G and gamma_occ against the oracle (its O6 loop is ~1e11 long-double operations: the slow test of this file)."""
+    o, v, naux = 129, 260, 16
+    spec = ClusterSpec(87, 0, o + v, o, v, naux, 40, "std")
+    x, info, out = _solve(spec, want=("E", "occ"))
+    assert info["general"] == 1
+    B = _oracle_B(x)
+    Gor = oracle.pair_G(B, x.e_occ, x.e_vir)
+    Eor = oracle.trace(x.P_frag, Gor)
+    assert abs(out["E"] - Eor) <= 1e-10 * abs(Eor)
+    _close(out["G"], Gor)
+    _close(out["occ"], oracle.rdm_occ(B, x.e_occ, x.e_vir))
