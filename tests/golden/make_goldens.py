@@ -113,7 +113,14 @@ def single(case, spec, cache, threads, jchunk, subset=0, want_gamma=False):
         C_vir, e_vir = np.ascontiguousarray(x.C_vir[:, virt]), np.ascontiguousarray(x.e_vir[virt])
     else:
         virt, C_vir, e_vir = None, x.C_vir, x.e_vir
-    B = _B(case, x, C_vir, cache, threads)
+    parent = os.path.join(cache, f"B_{case.rsplit('_v', 1)[0]}.npy") if subset else ""
+    if subset and os.path.exists(parent):
+        # B[i][a][P] of the kept columns is a slice of the parent case's oracle B (every (i,a,P) entry is its own sum over
+        # mu, nu in O2-O3: identical operations, identical bits) — saves repeating O1-O2 on all aux rows
+        B = np.ascontiguousarray(np.load(parent, mmap_mode="r")[:, virt, :])
+        _log(f"  {case}: B sliced from {os.path.basename(parent)}")
+    else:
+        B = _B(case, x, C_vir, cache, threads)
     G = _G(case, B, x.e_occ, e_vir, cache, jchunk)
     arrays = {"G": G}
     meta = {"case": case, "spec": _spec_meta(spec), "max_abs_G": float(np.max(np.abs(G))), **_energies(x, G)}
