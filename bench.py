@@ -628,11 +628,26 @@ def run_gpu(args) -> None:
 
     # ---- the other halves of the metric, time-boxed, same process / same timing: clusters/s of the 96-cluster batch
     #      (config 2) and the roofline fraction at each resident point of the size sweep (config 4)
-    batch, sweep = None, None
+    batch, sweep, next_rows = None, None, None
     if args.extras and gb.world == 1 and args.workload == "config3":
         k, w = max(1, min(args.steps, 3)), 3
         batch = gb.sub_object("config2", k, w)
         sweep = [gb.sub_object(f"config4:{i}", k, w) for i in range(3)]  # v = 256, 512, 1024 (v = 2048: --streamed)
+        # the rows next to the hot path, small time-boxed cases: both 1-RDM blocks and the rank-r energy on
+        # config 1; the general route (nocc > 128) on the environment-occupied x impurity-virtual shape; the canonical
+        # out-of-core energy with its B store in pinned host memory
+        next_rows = {}
+        for nm, wl in (("config1", "config1"), ("general_454x64", "custom:454,64,2072,32")):
+            mm = gb.measure(wl, 2, 2, want_e2e=False, want_rdm=True)
+            zz = gb.summarize(mm)
+            ent = dict(mm["next1"] or {}, workload=wl, energy_ms=zz["roofline"]["ms_per_launch"], energy_pair_frac=zz["roofline"]["frac"])
+            for kk in ("rdm_occ", "rdm_vir"):
+                if kk in ent:
+                    ent[kk]["frac_of_fp64_peak"] = ent[kk]["tflops"] / gb.peak if gb.peak else None
+            next_rows[nm] = ent
+        cm = canonical_measure("128,512,2560,32,host", 4.0)
+        next_rows["canonical_out_of_core"] = {kk: cm[kk] for kk in ("nocc", "nvir", "naux", "store", "info", "E_MP2", "transform_ms", "energy_ms",
+                                                                "energy_tflops", "energy_frac_of_fp64_peak", "panel_gbs")}
 
     # ---- CPU oracle beside it (rank 0, N = 1 only): bounded sample, extrapolated
     cpu = None
@@ -660,6 +675,7 @@ def run_gpu(args) -> None:
         if batch is not None:
             line["batch"] = batch
             line["sweep"] = sweep
+            line["next_rows"] = next_rows
         e2e = None
         if m["e2e"] is not None:
             ms_e2e = m["e2e"]["ms"]
@@ -738,15 +754,19 @@ def run_streamed(args) -> None:
 
 
 def run_canonical(args) -> None:
+    print(json.dumps(canonical_measure(args.canonical, args.stream_gb)))
+
+
+def canonical_measure(desc: str, stream_gb: float = 8.0) -> dict:
     """NEXT-2 (not a bench line): whole-system canonical DF-MP2 energy, B store in pinned host memory (out of core) or on the
-    device.  --canonical o,v,naux[,occ_block[,host|device]]; nao = o + v; the packed integrals are generated and fed in aux
+    device.  desc = o,v,naux[,occ_block[,host|device]]; nao = o + v; the packed integrals are generated and fed in aux
     blocks (never resident at once).  Reports the device time of the two phases (CUDA events) and the panel traffic."""
     import torch
 
     import paper_2412_18553_b200 as sie
 
     torch.cuda.set_device(0)
-    f = args.canonical.split(",")
+    f = desc.split(",")
     o, v, naux = int(f[0]), int(f[1]), int(f[2])
     occ_block = int(f[3]) if len(f) > 3 else 0
     store = f[4] if len(f) > 4 else "host"
@@ -755,7 +775,7 @@ def run_canonical(args) -> None:
     cu = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()  # noqa: E731
     s = sie.CanonicalSolver(spec.nao, o, v, naux, occ_block=occ_block, store=store)
     info = s.info()
-    blk = max(8, min(naux, int(args.stream_gb * 1e9) // (8 * spec.npair)) // 8 * 8)
+    blk = max(8, min(naux, int(stream_gb * 1e9) // (8 * spec.npair)) // 8 * 8)
     pinned = torch.empty((blk, spec.npair), dtype=torch.float64, pin_memory=True)
     Ld = torch.empty((blk, spec.npair), dtype=torch.float64, device="cuda")
     C_occ, C_vir, e_occ, e_vir = cu(x.C_occ), cu(x.C_vir), cu(x.e_occ), cu(x.e_vir)
@@ -794,7 +814,8 @@ def run_canonical(args) -> None:
             "panel_gbs": panel_bytes / (t_en * 1e-3) * 1e-9, "b_store_bytes": s.bstore_bytes, "workspace_bytes": s.workspace_bytes,
             "gpu_launches": sie.launch_count() - l0, "clocks": cs.summary(),
             "note": "device time of each phase (CUDA events); packed integrals generated and fed in aux blocks; data synthetic"}
-    print(json.dumps(line))
+    s.close()
+    return line
 
 
 def main() -> None:
