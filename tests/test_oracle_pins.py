@@ -253,3 +253,34 @@ def test_nmo_smaller_than_nao():
     F = _full_from_packed(Lp, x.spec.nao)
     B_np = np.einsum("mi,Pmn,na->iaP", x.C_occ, F, x.C_vir)
     assert np.max(np.abs(B - B_np)) <= 1e-14 * max(1.0, np.max(np.abs(B_np)))
+
+
+def test_P9_blas_route_agrees_with_the_loop_oracle_at_config1_scale():
+    """Pin P-9: a second CPU route — unpack with np.tril_indices, BLAS matmuls for both half transforms and
+    the pair integrals, vectorised G in plain doubles (different summation order everywhere) — agrees with the loop oracle
+    on the dense config-1 problem (o=30, v=270, nao=300, naux=1200) to ~1e-13 relative: the loop oracle's indexing holds
+    at a size with many aux blocks, ragged 8-wide dot tails and 72 900 virtual pairs per occupied pair."""
+    from workloads import config_specs, make_cluster
+
+    spec = config_specs(1)[0]
+    x = make_cluster(spec)
+    Lp = x.L_packed(threads=4)
+    o, v, nao, naux = spec.nocc, spec.nvir, spec.nao, spec.naux
+    iu = np.tril_indices(nao)
+    H = np.empty((naux, o, nao))
+    F = np.zeros((nao, nao))
+    for P in range(naux):  # H^P = C_occ^T L^P with L^P rebuilt from its packed row
+        F[iu] = Lp[P]
+        F.T[iu] = Lp[P]
+        H[P] = x.C_occ.T @ F
+    Bnp = np.ascontiguousarray(np.einsum("Pin,na->iaP", H, x.C_vir, optimize=True))  # [o][v][naux]
+    Bor = oracle.transform(x.C_occ, x.C_vir, Lp)
+    assert np.max(np.abs(Bnp - Bor)) <= 1e-13 * np.max(np.abs(Bor))
+    ovov = (Bnp.reshape(o * v, naux) @ Bnp.reshape(o * v, naux).T).reshape(o, v, o, v)  # (ia|jb)
+    D = x.e_occ[:, None, None, None] + x.e_occ[None, None, :, None] - x.e_vir[None, :, None, None] - x.e_vir[None, None, None, :]
+    t = ovov / D
+    W = 2.0 * ovov - ovov.transpose(0, 3, 2, 1)
+    Gnp = np.einsum("pajb,iajb->pi", t, W, optimize=True)
+    Gor = oracle.pair_G(Bor, x.e_occ, x.e_vir)
+    assert np.max(np.abs(Gnp - Gor)) <= 1e-12 * np.max(np.abs(Gor))
+    assert abs(np.einsum("ip,pi->", x.P_frag, Gnp) - oracle.trace(x.P_frag, Gor)) <= 1e-12 * abs(oracle.trace(x.P_frag, Gor))
