@@ -9,9 +9,11 @@
 //                     gamma_vir[a][c] += sum_{i,b,k} S1[a][(i,b,k)] S2[c][(i,b,k)]       Eq. S17 (L355), b the summed virtual
 //      split over K-ranges into partial slots that reduce_trace_kernel sums in fixed order (no atomics).
 //
-// The amplitude slab of one occupied block (<= 2 GB) is the only O(n^4)-shaped object and it lives for one block; nothing
-// of size o^2 v^2 exists.  The slab GEMM forms ordered pairs (i,k), i.e. twice the SYRK minimum of the fused kernel: this
-// is the general route, the fused kernel stays the fast one.
+// Block-slab mode: the amplitude slab of one occupied block (<= 1 GB, power-of-two block) is the only O(n^4)-shaped object
+// and it lives for one block; the slab GEMM forms ordered pairs (i,k), i.e. twice the SYRK minimum of the fused kernel.
+// Whole-matrix mode (general_geom().full: the integral matrix (o v)^2 doubles fits in 8 GB — the large-occ x small-vir
+// sub-space of the BNO step and every small cluster): one block covers the cluster and stage 1 is a SYRK (one job per
+// 128-row block from its diagonal on, lower triangle mirrored): the o^2 v^2 naux minimum.
 #include <algorithm>
 #include <cstring>
 #include <vector>

@@ -268,3 +268,35 @@ def test_general_route_block_slab_mode_large_integral_matrix():
     assert abs(out["E"] - Eor) <= 1e-10 * abs(Eor)
     _close(out["G"], Gor)
     _close(out["occ"], oracle.rdm_occ(B, x.e_occ, x.e_vir))
+
+
+def test_degenerate_sizes_of_the_next_rows():
+    """o = v = 1 closed forms through every route that has one (PAPER.md Eq. S15-S18 with a single amplitude t):
+    E = (ia|ia)^2 / (2 (e_i - e_a)), gamma_occ = 2 - 2 t^2, gamma_vir = 2 t^2; naux = 1; a one-row, one-column projector."""
+    rng = np.random.default_rng(11)
+    for naux in (1, 5):
+        spec = ClusterSpec(88, naux, 2, 1, 1, naux, 0, "std")
+        x = make_cluster(spec)
+        Lp = x.L_packed()
+        Bv = oracle.transform(x.C_occ, x.C_vir, Lp)[0, 0]
+        iaia = float(np.sum(Bv * Bv))
+        ei, ea = float(x.e_occ[0]), float(x.e_vir[0])
+        t = iaia / (2 * ei - 2 * ea)
+        s = sie.ClusterSolver(2, 1, 1, naux, flags=binding.SIE_FLAG_RDM_VIR)
+        s.transform(_cu(x.C_occ), _cu(x.C_vir), _cu(Lp), 0, naux)
+        e_occ, e_vir = _cu(x.e_occ), _cu(x.e_vir)
+        E, G = s.energy(e_occ, e_vir, None)
+        El = s.energy_lowrank(e_occ, e_vir, _cu(np.ones((1, 1))))
+        go, _ = s.rdm_occ(e_occ, e_vir)
+        gv, _ = s.rdm_vir(e_occ, e_vir)
+        torch.cuda.synchronize()
+        Ecf = iaia * iaia / (2 * (ei - ea))
+        for got in (float(E.cpu()[0]), float(El.cpu()[0]), float(G.cpu()[0, 0])):
+            assert abs(got - Ecf) <= 1e-12 * abs(Ecf)
+        assert abs(float(go.cpu()[0, 0]) - (2 - 2 * t * t)) <= 1e-13 and abs(float(gv.cpu()[0, 0]) - 2 * t * t) <= 1e-13 * max(1.0, 2 * t * t)
+        s.close()
+        c = sie.CanonicalSolver(2, 1, 1, naux, store="device")
+        c.transform(_cu(x.C_occ), _cu(x.C_vir), _cu(Lp), 0, naux)
+        Ec = float(c.energy(e_occ, e_vir).cpu()[0])
+        assert abs(Ec - Ecf) <= 1e-12 * abs(Ecf)
+        c.close()
