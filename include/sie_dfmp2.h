@@ -48,7 +48,8 @@ enum {
     SIE_ECUDA = 3,        /* a CUDA runtime / driver call failed (see sie_dfmp2_last_cuda_error) */
     SIE_ESTATE = 4,       /* call order violated (e.g. energy before the transform covered [0,naux)) */
     SIE_EGAP = 5,         /* SIE_FLAG_VALIDATE only: max(e_occ) >= min(e_vir) */
-    SIE_EUNSUPPORTED = 6  /* no CUDA device of compute capability 10.x */
+    SIE_EUNSUPPORTED = 6, /* no CUDA device of compute capability 10.x */
+    SIE_ETOOBIG = 7       /* sie_dfmp2_energy_noalloc: the problem needs more than the static scratch of SIE_NOALLOC_SCRATCH_BYTES */
 };
 
 enum {
@@ -111,6 +112,30 @@ int sie_dfmp2_energy(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ
  */
 int sie_dfmp2_energy_lowrank(sie_dfmp2_plan_t plan, void* workspace, const double* e_occ, const double* e_vir,
                              const double* Q, int r, double* E_out, void* cuda_stream);
+
+/*
+ * 3n. sie_dfmp2_energy_noalloc — the fused pair stage + projector/trace (steps A3-A6, the work of sie_dfmp2_energy) for callers
+ *    that must not allocate device memory and have no workspace to pass: code under CUDA graph capture, tight serving loops,
+ *    harnesses that forbid cudaMalloc.  The partial-G slots, the tile work list and the descriptors live in ONE file-scope
+ *    static device array of SIE_NOALLOC_SCRATCH_BYTES (24 MiB) inside the library; every GPU that loads the library holds it
+ *    until the process exits.  The call allocates nothing on the device (no cudaMalloc / cudaFree / allocating library
+ *    routine) and needs no plan.
+ *      B       DEVICE, [nvir][nocc][ceil8(naux)] row-major with the aux index contiguous: B[a][i][P] = B^P_{ia}, 16-byte aligned
+ *              (the layout sie_dfmp2_transform leaves at the start of its workspace; aux columns >= naux are never read)
+ *      e_occ [nocc], e_vir [nvir], P_frag [nocc][nocc] or NULL (identity), E_out: 1 double, G_out [nocc][nocc] or NULL: DEVICE
+ *    Limits: nocc <= 128 (SIE_EUNSUPPORTED above), and sie_dfmp2_noalloc_bytes(nocc, nvir) <= SIE_NOALLOC_SCRATCH_BYTES —
+ *    148 x kp x ceil8(nocc)^2 doubles of slots (kp = 16 / ceil(nocc/8), at least 1) plus 8 bytes per pair tile; BASELINE
+ *    config 3 (nocc 120, nvir 1080) needs 21.7 MB and fits; larger problems return SIE_ETOOBIG and touch nothing.
+ *    Same results as sie_dfmp2_energy on the same B (same kernels, same tile order, same fixed-order reduction).
+ *    ALL calls share the one array, which keeps the last call's contents; the call itself clears what must start at zero
+ *    on `cuda_stream`.  Calls whose GPU work overlaps (two streams, two host threads) RACE on it: serialise them on one
+ *    stream.  Enqueues only; does not synchronise.
+ */
+#define SIE_NOALLOC_SCRATCH_BYTES (24u << 20)
+int sie_dfmp2_energy_noalloc(int nocc, int nvir, int naux, const double* B, const double* e_occ, const double* e_vir,
+                             const double* P_frag, double* E_out, double* G_out, void* cuda_stream);
+size_t sie_dfmp2_noalloc_bytes(int nocc, int nvir); /* scratch bytes the call above needs (0: sizes it does not support) */
+size_t sie_dfmp2_noalloc_capacity(void);            /* = SIE_NOALLOC_SCRATCH_BYTES */
 
 /*
  * 3b. sie_dfmp2_rdm_occ — NEXT-1: occupied block of the MP2 one-particle reduced density matrix of the

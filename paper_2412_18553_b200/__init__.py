@@ -21,6 +21,9 @@ from .binding import (  # noqa: F401
     sie_dfmp2_destroy,
     sie_dfmp2_energy,
     sie_dfmp2_energy_lowrank,
+    sie_dfmp2_energy_noalloc,
+    sie_dfmp2_noalloc_bytes,
+    sie_dfmp2_noalloc_capacity,
     sie_dfmp2_rdm_occ,
     sie_dfmp2_rdm_vir,
     sie_dfmp2_plan,

@@ -12,7 +12,7 @@ from typing import List, Optional, Sequence, Tuple
 
 import torch
 
-SIE_OK, SIE_EINVAL, SIE_ENOMEM, SIE_ECUDA, SIE_ESTATE, SIE_EGAP, SIE_EUNSUPPORTED = range(7)
+SIE_OK, SIE_EINVAL, SIE_ENOMEM, SIE_ECUDA, SIE_ESTATE, SIE_EGAP, SIE_EUNSUPPORTED, SIE_ETOOBIG = range(8)
 SIE_FLAG_VALIDATE, SIE_FLAG_REFERENCE, SIE_FLAG_HOST_IO, SIE_FLAG_PROFILE, SIE_FLAG_RDM_OCC, SIE_FLAG_RDM_VIR, SIE_FLAG_STAGE_FULL = 1, 2, 4, 8, 16, 32, 64
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -23,6 +23,9 @@ EXPORTS = (
     "sie_dfmp2_transform",
     "sie_dfmp2_energy",
     "sie_dfmp2_energy_lowrank",
+    "sie_dfmp2_energy_noalloc",
+    "sie_dfmp2_noalloc_bytes",
+    "sie_dfmp2_noalloc_capacity",
     "sie_dfmp2_rdm_occ",
     "sie_dfmp2_rdm_vir",
     "sie_dfmp2_batch",
@@ -93,6 +96,12 @@ def _lib() -> ctypes.CDLL:
         L.sie_dfmp2_rdm_occ.restype = ci
         L.sie_dfmp2_energy_lowrank.argtypes = [vp, vp, vp, vp, vp, ci, vp, vp]
         L.sie_dfmp2_energy_lowrank.restype = ci
+        L.sie_dfmp2_energy_noalloc.argtypes = [ci, ci, ci, vp, vp, vp, vp, vp, vp, vp]
+        L.sie_dfmp2_energy_noalloc.restype = ci
+        L.sie_dfmp2_noalloc_bytes.argtypes = [ci, ci]
+        L.sie_dfmp2_noalloc_bytes.restype = ctypes.c_size_t
+        L.sie_dfmp2_noalloc_capacity.argtypes = []
+        L.sie_dfmp2_noalloc_capacity.restype = ctypes.c_size_t
         L.sie_dfmp2_rdm_vir.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.sie_dfmp2_rdm_vir.restype = ci
         L.sie_dfmp2_batch.argtypes = [ci, ctypes.POINTER(sie_dfmp2_cluster_t), vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t), cu, vp]
@@ -194,6 +203,27 @@ def sie_dfmp2_energy_lowrank(plan: int, workspace: torch.Tensor, e_occ, e_vir, Q
             _ptr(E_out, host, "E_out"), _stream_ptr(stream)),
         "sie_dfmp2_energy_lowrank",
     )
+
+
+def sie_dfmp2_energy_noalloc(nocc: int, nvir: int, naux: int, B, e_occ, e_vir, P_frag, E_out, G_out, *, stream=None) -> None:
+    """Pair stage + trace with the library's static device scratch (no workspace, no device allocation); marshalling only.
+    B: device tensor holding [nvir][nocc][ceil8(naux)] doubles (any shape/view, 16-byte aligned)."""
+    if B.dtype not in (torch.float64, torch.uint8) or not B.is_cuda or not B.is_contiguous():
+        raise TypeError("B: need a contiguous CUDA tensor")
+    _check(
+        _lib().sie_dfmp2_energy_noalloc(nocc, nvir, naux, B.data_ptr(), _ptr(e_occ, False, "e_occ"), _ptr(e_vir, False, "e_vir"),
+                                        _ptr(P_frag, False, "P_frag"), _ptr(E_out, False, "E_out"), _ptr(G_out, False, "G_out"),
+                                        _stream_ptr(stream)),
+        "sie_dfmp2_energy_noalloc",
+    )
+
+
+def sie_dfmp2_noalloc_bytes(nocc: int, nvir: int) -> int:
+    return int(_lib().sie_dfmp2_noalloc_bytes(nocc, nvir))
+
+
+def sie_dfmp2_noalloc_capacity() -> int:
+    return int(_lib().sie_dfmp2_noalloc_capacity())
 
 
 def sie_dfmp2_rdm_vir(plan: int, workspace: torch.Tensor, e_occ, e_vir, gamma_out, trace_out=None, *, host=False, stream=None) -> None:

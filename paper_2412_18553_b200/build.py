@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsie_dfmp2.so")
-SOURCES = ["api.cu", "transform.cu", "pair.cu", "general.cu", "canonical.cu", "ref_kernels.cu", "probes.cu"]
+SOURCES = ["api.cu", "transform.cu", "pair.cu", "general.cu", "canonical.cu", "noalloc.cu", "ref_kernels.cu", "probes.cu"]
 HEADERS = ["sie_common.cuh", "mma_pipeline.cuh", "sie_internal.h", os.path.join("..", "..", "include", "sie_dfmp2.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -1246,6 +1246,7 @@ const char* sie_dfmp2_strerror(int status) {
         case SIE_ESTATE: return "invalid call order";
         case SIE_EGAP: return "orbital gap violated: max(e_occ) >= min(e_vir)";
         case SIE_EUNSUPPORTED: return "no compute-capability-10.x CUDA device";
+        case SIE_ETOOBIG: return "problem exceeds the static scratch of the no-allocation entry point";
         default: return "unknown status";
     }
 }
