@@ -31,14 +31,19 @@ namespace sie {
 // Operand feed, two K-blocks of 8 per stage (one barrier round trip per 16 k values), each as dense [row][8] lines of 64 B (conflict-free LDS.128, see mma_pipeline.cuh):
 //   * A and the TMA-mode Bop: cp.async.bulk.tensor boxes {8, rows, 1}, completion by complete_tx on the stage's `full`.
 //   * the packed Bop: (P|mu nu) is stored as lower triangles, row mu at offset mu(mu+1)/2 — only 8-byte aligned and not
-//     a TMA tensor, so two producer warps gather it with 8-byte cp.async straight from the packed array: element
+//     a TMA tensor, so the producer warps gather it with 8-byte cp.async straight from the packed array: element
 //     (n = (P,nu), k = mu) comes from Lp[P][max(mu,nu)(max+1)/2 + min(mu,nu)].  Below the diagonal that is 64 contiguous
 //     bytes per row, above it 32-byte runs of 4 consecutive nu; the shared-memory side is always 256 contiguous bytes per
 //     warp instruction.  Completion by cp.async.mbarrier.arrive.noinc on the same `full` barrier.  The square
 //     (P|mu nu) is never materialised: every packed element is read by the two output tiles that need it, close together
 //     in time (the tiles of one P are consecutive in the work list), so it comes from HBM once and from L2 once.
 constexpr int XG_NCONS = 8;                 // consumer warps (2 x 4)
-constexpr int XG_NPROD = 2;                 // producer warps
+#ifndef SIE_XG_NPROD
+#define SIE_XG_NPROD 4
+#endif
+constexpr int XG_NPROD = SIE_XG_NPROD;      // producer warps (4: at small M the gather's address arithmetic is issue-bound on 2)
+constexpr int XG_RG = XG_NPROD * 4;         // row groups of the packed gather: thread (k, rg) owns column k of rows rg, rg + XG_RG, ...
+constexpr int XG_RPT = 128 / XG_RG;         // rows per producer thread and K-block
 constexpr int XG_THREADS = (XG_NCONS + XG_NPROD) * 32;
 constexpr int XG_TN = 128, XG_KB = 8, XG_TMMAX = 128;
 constexpr int XG_NSUB = 2;                  // K-blocks per pipeline stage: one full/empty barrier round trip per 16 k values
@@ -133,11 +138,11 @@ __global__ void __launch_bounds__(XG_THREADS, 1) xform_gemm_kernel(const XJob* _
                 // the 16 rows (P, nu) of this thread: offset of the packed row of nu, and of the matrix of P
                 const int nao = J->nao;
                 const long long npair = J->npair;
-                long long rowoff[16], matoff[16];
-                int nu[16];
+                long long rowoff[XG_RPT], matoff[XG_RPT];
+                int nu[XG_RPT];
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const long long n = (long long)nb * XG_TN + rg + 8 * j;
+                for (int j = 0; j < XG_RPT; ++j) {
+                    const long long n = (long long)nb * XG_TN + rg + XG_RG * j;
                     const bool ok = n < J->n_total;
                     const unsigned P = ok ? (unsigned)n / (unsigned)nao : 0u;  // the host keeps n_total below 2^31
                     nu[j] = ok ? (int)((unsigned)n - P * (unsigned)nao) : -1;  // -1: row past the end, zero filled
@@ -162,10 +167,10 @@ __global__ void __launch_bounds__(XG_THREADS, 1) xform_gemm_kernel(const XJob* _
                         const bool kok = mu < nao;
                         const uint32_t dst = smem_u32(s + u * XG_SUB_DOUBLES + XG_TMMAX * XG_KB) + 8u * (uint32_t)(rg * XG_KB + k);
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
+                        for (int j = 0; j < XG_RPT; ++j) {
                             const long long off = mu <= nu[j] ? rowoff[j] + mu : matoff[j] + trimu + nu[j];
                             const bool ok = kok && nu[j] >= 0;
-                            cp_async_8(dst + (uint32_t)(8 * j * XG_KB * 8), Lp + (ok ? off : 0), ok);
+                            cp_async_8(dst + (uint32_t)(XG_RG * j * XG_KB * 8), Lp + (ok ? off : 0), ok);
                         }
                     }
                     cp_async_arrive_noinc(&full[ps.stage]);
