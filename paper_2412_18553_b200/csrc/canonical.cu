@@ -160,7 +160,7 @@ int sie_dfmp2_canonical_plan(sie_dfmp2_canon_t* plan, int nao, int nocc, int nvi
     p->Ib = Ib;
     p->ldv = (long long)align_up((size_t)Ib * nvir, 8);
     p->panel_bytes = align_up((size_t)Ib * nvir * p->naux_ld * 8, 256);
-    p->max_jobs = 4;
+    p->max_jobs = 4 + (int)(((long long)Ib * nvir + 127) / 128);  // + one SYRK job per 128-row block of a diagonal block pair
     Carve c;
     p->off_CoT = c.take((size_t)nocc * p->nao_ld * 8);
     p->off_CvT = c.take((size_t)nvir * p->nao_ld * 8);
@@ -266,13 +266,35 @@ int sie_dfmp2_canonical_energy(sie_dfmp2_canon_t plan, void* workspace, const do
                 CAN_CUDA(cudaStreamWaitEvent(st, p.ev_ready[buf], 0));
                 PK = panel[1 + buf];
             }
-            XJob J;
-            GemmOut ov{};
-            ov.base = V, ov.ld_m = p.ldv, ov.M = ni * p.v, ov.inner = (int)p.ldv, ov.valid_inner = nk * p.v, ov.stride_outer = 0;
-            ov.n_lin_total = (long long)nk * p.v;
-            CAN_TRY(gemm_job(J, panel[0], (long long)ni * p.v, PK, (long long)nk * p.v, p.naux, p.naux_ld, ov));
-            CAN_CUDA(cudaMemcpyAsync(arena, &J, sizeof J, cudaMemcpyHostToDevice, st));
-            CAN_TRY(launch_xform_gemm(false, reinterpret_cast<const XJob*>(arena), 1, J.m_tiles * J.n_tiles, p.num_sms, st));
+            if (K == I) {
+                // diagonal block pair: V = B_I B_I^T is symmetric — a SYRK: one job per 128-row block from its diagonal on, then
+                // the lower triangle is mirrored (half the flops of the full block)
+                const long long rows = (long long)ni * p.v;
+                const int nrb = (int)((rows + 127) / 128);
+                std::vector<XJob> jobs((size_t)nrb);
+                long long t = 0;
+                for (int r = 0; r < nrb; ++r) {
+                    const long long r0 = (long long)r * 128, M = std::min<long long>(128, rows - r0), N = rows - r0;
+                    GemmOut ov{};
+                    ov.base = V + r0 * p.ldv + r0, ov.ld_m = p.ldv, ov.M = (int)M, ov.inner = (int)p.ldv, ov.valid_inner = (int)N, ov.stride_outer = 0;
+                    ov.n_lin_total = N;
+                    const double* Br = panel[0] + r0 * p.naux_ld;
+                    CAN_TRY(gemm_job(jobs[r], Br, M, Br, N, p.naux, p.naux_ld, ov));
+                    jobs[r].tile_begin = (int)t;
+                    t += (long long)jobs[r].m_tiles * jobs[r].n_tiles;
+                }
+                CAN_CUDA(cudaMemcpyAsync(arena, jobs.data(), jobs.size() * sizeof(XJob), cudaMemcpyHostToDevice, st));
+                CAN_TRY(launch_xform_gemm(false, reinterpret_cast<const XJob*>(arena), nrb, (int)t, p.num_sms, st));
+                CAN_TRY(launch_mirror_lower(V, rows, p.ldv, st));
+            } else {
+                XJob J;
+                GemmOut ov{};
+                ov.base = V, ov.ld_m = p.ldv, ov.M = ni * p.v, ov.inner = (int)p.ldv, ov.valid_inner = nk * p.v, ov.stride_outer = 0;
+                ov.n_lin_total = (long long)nk * p.v;
+                CAN_TRY(gemm_job(J, panel[0], (long long)ni * p.v, PK, (long long)nk * p.v, p.naux, p.naux_ld, ov));
+                CAN_CUDA(cudaMemcpyAsync(arena, &J, sizeof J, cudaMemcpyHostToDevice, st));
+                CAN_TRY(launch_xform_gemm(false, reinterpret_cast<const XJob*>(arena), 1, J.m_tiles * J.n_tiles, p.num_sms, st));
+            }
             if (buf >= 0) CAN_CUDA(cudaEventRecord(p.ev_free[buf], st));
             canonical_energy_kernel<<<CAN_GRID, 256, 0, st>>>(V, ni, nk, p.v, p.ldv, e_occ + i0, e_occ + k0, e_vir, K == I ? 1.0 : 2.0, slots);
             note_launch();

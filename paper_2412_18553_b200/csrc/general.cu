@@ -66,6 +66,14 @@ __global__ void mirror_lower_kernel(double* __restrict__ V, long long n, long lo
     }
 }
 
+int launch_mirror_lower(double* V, long long n, long long ld, cudaStream_t st) {
+    const unsigned nb32 = (unsigned)((n + 31) / 32);
+    mirror_lower_kernel<<<dim3(nb32, nb32), dim3(32, 8), 0, st>>>(V, n, ld);
+    note_launch();
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SIE_OK : set_cuda_error(e);
+}
+
 GeneralGeom general_geom(int o, int v, int num_sms) {
     GeneralGeom g{};
     int Kb = 1;

@@ -105,6 +105,9 @@ size_t general_scratch_bytes(const GeneralGeom& g, int o);
 int general_pair(const GeneralGeom& g, const double* Bmat, int o, int v, int naux, int naux_ld, const double* e_occ, const double* e_vir,
                  int mode, unsigned char* scratch, double* slots, int* nslots, int num_sms, cudaStream_t st);
 
+// V[r][c] = V[c][r] for r > c of a square n x n matrix (leading dimension ld) whose upper triangle was computed
+int launch_mirror_lower(double* V, long long n, long long ld, cudaStream_t st);
+
 // ---- ref_kernels.cu ----------------------------------------------------------------------------
 // Simple FP64-FMA kernels following the definition step by step (any nocc). B layout [v][o][naux_ld].
 int ref_transform(const double* C_occ, const double* C_vir, const double* Lp_block, int nao, int o, int v, int p0, int p1,
