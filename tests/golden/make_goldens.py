@@ -13,6 +13,9 @@ Cases (BASELINE.json configs; generator recipe in workloads/gen.py):
   config4_k      sweep point k (o=64, v=256/512/1024/2048): G, E_frag (rank 32), E(P=I); gamma_occ for k <= 1
   config4_3_v256 the v=2048 point (nao=2112, naux=8448, packed integrals 150.8 GB) with C_vir zeroed outside 256 seeded
                  columns: the compressed problem for the oracle, the full-size streamed launch for the GPU; G, E, gamma_occ
+  config4_3_o8   the same v=2048 point with all 2048 virtuals and all 8448 aux rows dense and C_occ zeroed outside
+                 workloads.occupied_subset(spec, 8): the 8 x 8 block of G and gamma_occ on the kept occupieds, E_frag with
+                 the matching block of P_frag, E(P=I)
 
 What is computed is exactly oracle.transform_block (O1-O3), oracle.pair_G (O4-O6) and oracle.trace (O7) as they
 stand.  The only thing this script adds is bookkeeping: the aux index is fed in blocks (the oracle's own p0/p1
@@ -39,25 +42,25 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 import oracle  # noqa: E402
-from workloads import config_specs, make_cluster, virtual_subset  # noqa: E402
+from workloads import config_specs, make_cluster, occupied_subset, virtual_subset  # noqa: E402
 
 
 def _log(msg):
     print(time.strftime("%H:%M:%S"), msg, flush=True)
 
 
-def _B(case, x, C_vir, cache, threads, pblk=96):
-    """O1-O3 in aux blocks; B [nocc][nvir'][naux]."""
+def _B(case, x, C_occ, C_vir, cache, threads, pblk=96):
+    """O1-O3 in aux blocks; B [nocc'][nvir'][naux]."""
     spec = x.spec
     path = os.path.join(cache, f"B_{case}.npy")
     if os.path.exists(path):
         return np.load(path)
-    B = np.zeros((spec.nocc, C_vir.shape[1], spec.naux))
+    B = np.zeros((C_occ.shape[1], C_vir.shape[1], spec.naux))
     buf = np.empty((pblk, spec.npair))
     for p0 in range(0, spec.naux, pblk):
         p1 = min(spec.naux, p0 + pblk)
         Lb = x.L_block(p0, p1, out=buf[: p1 - p0], threads=threads)
-        oracle.transform_block(x.C_occ, C_vir, Lb, p0, p1, B)
+        oracle.transform_block(C_occ, C_vir, Lb, p0, p1, B)
         if (p0 // pblk) % 10 == 0:
             _log(f"  {case}: transform rows {p1}/{spec.naux}")
     if B.nbytes > (64 << 20):
@@ -85,8 +88,8 @@ def _G(case, B, e_occ, e_vir, cache, jchunk):
     return np.asarray(acc, dtype=np.float64)
 
 
-def _energies(x, G):
-    return {"E_frag": oracle.trace(x.P_frag, G), "E_identity": oracle.trace(None, G)}
+def _energies(P_frag, G):
+    return {"E_frag": oracle.trace(P_frag, G), "E_identity": oracle.trace(None, G)}
 
 
 def _write(case, arrays, meta):
@@ -105,7 +108,7 @@ def _spec_meta(spec):
             "nvir": spec.nvir, "naux": spec.naux, "rank": spec.rank, "scale": spec.scale}
 
 
-def single(case, spec, cache, threads, jchunk, subset=0, want_gamma=False):
+def single(case, spec, cache, threads, jchunk, subset=0, want_gamma=False, occ_subset=0):
     t0 = time.time()
     x = make_cluster(spec)
     if subset:
@@ -113,6 +116,11 @@ def single(case, spec, cache, threads, jchunk, subset=0, want_gamma=False):
         C_vir, e_vir = np.ascontiguousarray(x.C_vir[:, virt]), np.ascontiguousarray(x.e_vir[virt])
     else:
         virt, C_vir, e_vir = None, x.C_vir, x.e_vir
+    C_occ, e_occ, P_frag, occ = x.C_occ, x.e_occ, x.P_frag, None
+    if occ_subset:  # zero columns of C_occ give zero rows of B: their pairs contribute nothing to any sum (numerators are 0)
+        occ = occupied_subset(spec, occ_subset)
+        C_occ, e_occ = np.ascontiguousarray(x.C_occ[:, occ]), np.ascontiguousarray(x.e_occ[occ])
+        P_frag = np.ascontiguousarray(x.P_frag[np.ix_(occ, occ)])
     parent = os.path.join(cache, f"B_{case.rsplit('_v', 1)[0]}.npy") if subset else ""
     if subset and os.path.exists(parent):
         # B[i][a][P] of the kept columns is a slice of the parent case's oracle B (every (i,a,P) entry is its own sum over
@@ -120,15 +128,18 @@ def single(case, spec, cache, threads, jchunk, subset=0, want_gamma=False):
         B = np.ascontiguousarray(np.load(parent, mmap_mode="r")[:, virt, :])
         _log(f"  {case}: B sliced from {os.path.basename(parent)}")
     else:
-        B = _B(case, x, C_vir, cache, threads)
-    G = _G(case, B, x.e_occ, e_vir, cache, jchunk)
+        B = _B(case, x, C_occ, C_vir, cache, threads)
+    G = _G(case, B, e_occ, e_vir, cache, jchunk)
     arrays = {"G": G}
-    meta = {"case": case, "spec": _spec_meta(spec), "max_abs_G": float(np.max(np.abs(G))), **_energies(x, G)}
+    meta = {"case": case, "spec": _spec_meta(spec), "max_abs_G": float(np.max(np.abs(G))), **_energies(P_frag, G)}
+    if occ_subset:
+        arrays["occupied_subset"] = occ
+        meta["occupied_subset"] = int(occ_subset)
     if subset:
         arrays["virtual_subset"] = virt
         meta["virtual_subset"] = int(subset)
     if want_gamma:
-        g = oracle.rdm_occ(B, x.e_occ, e_vir)
+        g = oracle.rdm_occ(B, e_occ, e_vir)
         arrays["gamma_occ"] = g
         meta["trace_gamma_occ"] = float(np.trace(g))
     meta["oracle_threads"] = oracle.threads()
@@ -182,6 +193,8 @@ def main():
             single(case, config_specs(3)[0], a.cache, a.threads, a.jchunk, subset=256, want_gamma=True)
         elif case == "config4_3_v256":
             single(case, config_specs(4)[6], a.cache, a.threads, a.jchunk, subset=256, want_gamma=True)
+        elif case == "config4_3_o8":
+            single(case, config_specs(4)[6], a.cache, a.threads, a.jchunk, want_gamma=True, occ_subset=8)
         elif case.startswith("config4_"):
             k = int(case.split("_")[1])
             single(case, config_specs(4)[2 * k], a.cache, a.threads, a.jchunk, want_gamma=(k <= 1))

@@ -19,7 +19,7 @@ import pytest
 import torch
 
 import paper_2412_18553_b200 as sie
-from workloads import config_specs, make_cluster, virtual_subset
+from workloads import config_specs, make_cluster, occupied_subset, virtual_subset
 
 pytestmark = pytest.mark.gpu
 
@@ -146,21 +146,31 @@ def test_config3_dense_aux_256_dense_virtuals_matches_golden(config3_inputs):
 
 
 # ---------------------------------------------------------------------------------------------- config 4: the size sweep
-@pytest.mark.parametrize("k", [0, 1, 2, 3, "3_v256"])
+@pytest.mark.parametrize("k", [0, 1, 2, 3, "3_v256", "3_o8"])
 def test_config4_sweep_point_matches_golden(k):
     """k = "3_v256": the v = 2048 point with C_vir zeroed outside 256 seeded columns (dense aux, dense occupied): the GPU
-    streams all 150.8 GB of packed integrals and runs the full-size launch, the oracle ran the compressed problem."""
+    streams all 150.8 GB of packed integrals and runs the full-size launch, the oracle ran the compressed problem.
+    k = "3_o8": the same point with all 2048 virtuals and all 8448 aux rows dense and C_occ zeroed outside 8 seeded columns:
+    every virtual-pair tile of the full-size launch carries non-zeros; the 8 x 8 block of G on the kept occupieds is the
+    oracle's compressed problem, the rest of G is exactly zero (zero rows of B give zero integrals and amplitudes)."""
     meta, arr = _golden(f"config4_{k}")
-    sub = isinstance(k, str)
+    sub = k if isinstance(k, str) else ""
     k = 3 if sub else k
     spec = config_specs(4)[2 * k]  # rank-32 projector; the P = I run shares G (A-15)
     x = make_cluster(spec)
-    if sub:
+    occ = None
+    if sub == "3_v256":
         virt = virtual_subset(spec, 256)
         assert np.array_equal(virt, arr["virtual_subset"])
         Cz = np.zeros_like(x.C_vir)
         Cz[:, virt] = x.C_vir[:, virt]
         x.C_vir = Cz
+    elif sub == "3_o8":
+        occ = occupied_subset(spec, 8)
+        assert np.array_equal(occ, arr["occupied_subset"])
+        Cz = np.zeros_like(x.C_occ)
+        Cz[:, occ] = x.C_occ[:, occ]
+        x.C_occ = Cz
     _need_gb(8 * spec.naux * spec.npair / 2**30 + 16 if k < 3 else 40)
     s = sie.ClusterSolver(spec.nao, spec.nocc, spec.nvir, spec.naux)
     C_occ, C_vir = _cu(x.C_occ), _cu(x.C_vir)
@@ -184,10 +194,24 @@ def test_config4_sweep_point_matches_golden(k):
     torch.cuda.synchronize()
     _assert_E(float(E.cpu()[0]), meta["E_frag"])
     _assert_E(float(E_I.cpu()[0]), meta["E_identity"])
-    _assert_G(G.cpu().numpy(), arr["G"])
+    Gh = G.cpu().numpy()
+    if occ is not None:  # everything outside the kept block is exactly zero; the block is the oracle's compressed problem
+        mask = np.ones_like(Gh, dtype=bool)
+        mask[np.ix_(occ, occ)] = False
+        assert not np.any(Gh[mask])
+        Gh = Gh[np.ix_(occ, occ)]
+    _assert_G(Gh, arr["G"])
     if "gamma_occ" in arr.files:
         gam, _ = s.rdm_occ(e_occ, e_vir)
-        _assert_G(gam.cpu().numpy(), arr["gamma_occ"])
+        gh = gam.cpu().numpy()
+        if occ is not None:  # untouched occupieds keep occupation 2 exactly (Eq. S18 with zero amplitudes)
+            rest = gh.copy()
+            rest[np.ix_(occ, occ)] = 0.0
+            expect = 2.0 * np.eye(spec.nocc)
+            expect[np.ix_(occ, occ)] = 0.0
+            assert np.array_equal(rest, expect)
+            gh = gh[np.ix_(occ, occ)]
+        _assert_G(gh, arr["gamma_occ"])
     s.close()
     del L
     torch.cuda.empty_cache()

@@ -10,5 +10,6 @@ from .gen import (  # noqa: F401
     config_specs,
     make_cluster,
     npair,
+    occupied_subset,
     virtual_subset,
 )

@@ -23,7 +23,7 @@ from typing import List, Optional
 import numpy as np
 
 # stream ids inside SeedSequence([config_id, cluster_id, stream_id])
-_S_C, _S_EOCC, _S_EVIR, _S_Q, _S_NOCC, _S_SUBSET = 1, 2, 3, 4, 5, 6
+_S_C, _S_EOCC, _S_EVIR, _S_Q, _S_NOCC, _S_SUBSET, _S_OSUBSET = 1, 2, 3, 4, 5, 6, 7
 _S_L0 = 100  # aux index P uses stream 100 + P
 
 
@@ -122,6 +122,15 @@ def virtual_subset(spec: ClusterSpec, k: int) -> np.ndarray:
     r = _rng(spec, _S_SUBSET)
     inner = r.choice(np.arange(1, spec.nvir - 1), size=k - 2, replace=False)
     return np.sort(np.concatenate([[0, spec.nvir - 1], inner])).astype(np.int64)
+
+
+def occupied_subset(spec: ClusterSpec, k: int) -> np.ndarray:
+    """Sorted, seeded choice of ``k`` of the ``nocc`` occupied columns, always containing the first and the last one
+    (the "dense aux x dense virtuals x k dense occupieds" full-size parity case: C_occ is zeroed outside these columns)."""
+    assert 2 <= k <= spec.nocc
+    r = _rng(spec, _S_OSUBSET)
+    inner = r.choice(np.arange(1, spec.nocc - 1), size=k - 2, replace=False)
+    return np.sort(np.concatenate([[0, spec.nocc - 1], inner])).astype(np.int64)
 
 
 def make_cluster(spec: ClusterSpec) -> ClusterInputs:
