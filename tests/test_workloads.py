@@ -49,3 +49,17 @@ def test_L_blocks_are_blocking_independent_and_scaled():
     assert abs(Lb.std() * np.sqrt(100) - 1.0) < 0.02  # variance 1/nao
     Ls = make_cluster(ClusterSpec(7, 4, 100, 10, 90, 40, 2, "std")).L_packed()
     assert np.allclose(Ls * 10.0, Lb)  # std 1/nao variant is the same draw rescaled
+
+
+def test_orbital_subsets_are_seeded_sorted_and_keep_both_ends():
+    """The column subsets of the 'dense aux x k dense virtuals / occupieds' full-size goldens."""
+    from workloads import occupied_subset, virtual_subset
+
+    spec = config_specs(4)[6]
+    for pick, n, k in ((virtual_subset, spec.nvir, 256), (occupied_subset, spec.nocc, 8)):
+        s = pick(spec, k)
+        assert s.dtype == np.int64 and s.shape == (k,) and np.array_equal(s, pick(spec, k))
+        assert s[0] == 0 and s[-1] == n - 1 and np.all(np.diff(s) > 0)
+    # independent streams: the two choices of one spec are not prefixes of one another, other clusters draw other columns
+    assert not np.array_equal(occupied_subset(spec, 8), virtual_subset(spec, 8))
+    assert not np.array_equal(occupied_subset(spec, 8), occupied_subset(config_specs(4)[4], 8))
