@@ -23,20 +23,57 @@ namespace sie {
 
 constexpr int CAN_GRID = 1184;  // 148 x 8 CTAs of the energy pass, each with a private partial-sum slot
 
-// V [(i,a)][(k,b)] with leading dimension ldv; rows i in [0,ni), columns k in [0,nk); e_i / e_k point at the blocks' energies
+// V [(i,a)][(k,b)] with leading dimension ldv; rows i in [0,ni), columns k in [0,nk); e_i / e_k point at the blocks' energies.
+// The exchange partner (ib|ka) of an element is its transpose INSIDE the v x v block of one (i,k) pair, so the block is walked
+// in pairs of 32 x 32 tiles (ta <= tb): both tiles are read once with coalesced rows, the transposed operand comes from
+// shared memory, and one tile pair yields the terms of (a,b) and of (b,a) — V is read from HBM exactly once (an
+// element-wise walk fetched a 32-byte sector for every 8-byte partner: 4.5x the bytes).
 __global__ void __launch_bounds__(256) canonical_energy_kernel(const double* __restrict__ V, int ni, int nk, int v, long long ldv,
                                                                 const double* __restrict__ e_i, const double* __restrict__ e_k,
                                                                 const double* __restrict__ e_vir, double weight, double* __restrict__ slots) {
-    const long long ncol = (long long)nk * v, total = (long long)ni * v * ncol;
+    __shared__ double T1[32][33], T2[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int nt = (v + 31) / 32;
+    const long long ntp = (long long)nt * (nt + 1) / 2, total = (long long)ni * nk * ntp;
     double s = 0.0;
-    for (long long e = blockIdx.x * 256LL + threadIdx.x; e < total; e += (long long)gridDim.x * 256) {
-        const long long row = e / ncol, col = e - row * ncol;
-        const int i = (int)(row / v), a = (int)(row - (long long)i * v);
-        const int k = (int)(col / v), b = (int)(col - (long long)k * v);
-        const double x = V[row * ldv + col];
-        const double y = V[((long long)i * v + b) * ldv + (long long)k * v + a];  // (ib|ka)
-        const double D = ((e_i[i] + e_k[k]) - e_vir[a]) - e_vir[b];
-        s += x * fma(2.0, x, -y) / D;
+    for (long long item = blockIdx.x; item < total; item += gridDim.x) {
+        const long long ik = item / ntp;
+        int rem = (int)(item - ik * ntp), ta = 0;
+        while (rem >= nt - ta) {
+            rem -= nt - ta;
+            ++ta;
+        }
+        const int tb = ta + rem;
+        const int i = (int)(ik / nk), k = (int)(ik - (long long)i * nk);
+        const int a0 = 32 * ta, b0 = 32 * tb;
+        const double* blk = V + (long long)i * v * ldv + (long long)k * v;  // V_ik [a][b], row stride ldv
+#pragma unroll
+        for (int r = ty; r < 32; r += 8) {
+            const bool in1 = a0 + r < v && b0 + tx < v, in2 = b0 + r < v && a0 + tx < v;
+            T1[r][tx] = in1 ? blk[(long long)(a0 + r) * ldv + b0 + tx] : 0.0;
+            T2[r][tx] = (ta != tb && in2) ? blk[(long long)(b0 + r) * ldv + a0 + tx] : 0.0;
+        }
+        __syncthreads();
+        const double eik = e_i[i] + e_k[k];
+        const int b = b0 + tx;
+        if (b < v) {
+            const double eb = e_vir[b];
+#pragma unroll
+            for (int r = ty; r < 32; r += 8) {
+                const int a = a0 + r;
+                if (a >= v) break;
+                const double D = (eik - e_vir[a]) - eb;
+                const double x = T1[r][tx];
+                if (ta == tb) {
+                    const double y = T1[tx][r];  // (ib|ka) of the same tile
+                    s += x * fma(2.0, x, -y) / D;
+                } else {
+                    const double y = T2[tx][r];  // element (b,a) of the block: the (a,b) term and the (b,a) term share D
+                    s += (x * fma(2.0, x, -y) + y * fma(2.0, y, -x)) / D;
+                }
+            }
+        }
+        __syncthreads();
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
