@@ -725,7 +725,7 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
             ProfSpan ps(p.prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc),
                                 reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8,
-                                (mode == 0 && o <= 64) ? 3 : mode, st));
+                                (mode == 0 && o <= PAIR_SMALL_STRIP_MAX_O) ? 3 : mode, st));
         }
         rc.gpart = gpart;
         rc.o8 = p.o8;
@@ -1160,7 +1160,7 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_CUDA(cudaMemsetAsync(ws + off_tiles + tiles.size() * sizeof(PairTile), 0, 256, st));
             ProfSpan ps(prof, ST_PAIR, st);
             bool any_small = false;
-            for (int k : order) any_small = any_small || plans[k].o <= 64;
+            for (int k : order) any_small = any_small || plans[k].o <= PAIR_SMALL_STRIP_MAX_O;
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
                                 (int)tiles.size(), ncta, tmax, (mode == 0 && any_small) ? 3 : mode, st));
         }

@@ -71,6 +71,10 @@ struct PairGeom {                  // tile configuration facts for host-side pla
     int TM, TN, ncons;
 };
 PairGeom pair_geom();
+// Energy-mode launches that contain a cluster with nocc <= this use the kernel instantiation whose strips of such clusters
+// are epilogue_strip_small (launch_pair mode 3).  Measured (custom:o,4o,1536): small strips +4...5.5 % at o = 72...96,
+// -1 % at 104, -5 % at 112, -6 % at 120, equal at 128 — so larger blocks keep the generic strip in either instantiation.
+constexpr int PAIR_SMALL_STRIP_MAX_O = 96;
 size_t pair_smem_bytes();
 // mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma), 2 energy only with a low-rank projector, 3 = mode 0 through the
 // instantiation whose strips for o <= 64 are epilogue_strip_small (same sums; chosen by the caller when such clusters exist); one mode per launch
