@@ -78,7 +78,13 @@ constexpr int PAIR_SMALL_STRIP_MAX_O = 96;
 size_t pair_smem_bytes();
 // mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma), 2 energy only with a low-rank projector, 3 = mode 0 through the
 // instantiation whose strips for o <= 64 are epilogue_strip_small (same sums; chosen by the caller when such clusters exist); one mode per launch
-int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, int mode, cudaStream_t st);
+// producer_warp: the math warp whose lane 0 issues the TMA loads (pair_producer_warp() for a tile edge t8)
+int launch_pair(const PairCluster* d_clusters, const PairTile* d_tiles, int ntiles, int ncta, int tmax, int mode, int producer_warp,
+                cudaStream_t st);
+// Tile edges that are not a multiple of 32 rows give the 4 x 4 warp grid uneven rectangles: warp 12 = (3,3) then owns the
+// smallest one and runs ahead of the others, which is where the producer lane belongs (it refills while it waits for its
+// own data); with even rectangles every warp has the same work and the producer stays on warp 0, topping up once per step.
+inline int pair_producer_warp(int t8) { return ((t8 >> 3) & 3) ? 12 : 0; }
 
 struct ReduceCluster {             // per cluster, device array
     const double* gpart;           // [nslots][o8*o8]
