@@ -725,7 +725,7 @@ static int energy_impl(sie_dfmp2_plan_t plan, void* workspace, const double* e_o
             ProfSpan ps(p.prof, ST_PAIR, st);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + p.off_desc),
                                 reinterpret_cast<const PairTile*>(ws + p.off_tiles), (int)p.tiles.size(), p.ncta, p.t8,
-                                (mode == 0 && o <= PAIR_SMALL_STRIP_MAX_O) ? 3 : mode, pair_producer_warp(p.t8), st));
+                                (mode == 0 && pair_small_strip(o, pair_producer_warp(p.t8) != 0)) ? 3 : mode, pair_producer_warp(p.t8), st));
         }
         rc.gpart = gpart;
         rc.o8 = p.o8;
@@ -1159,14 +1159,15 @@ int sie_dfmp2_batch(int ncluster, const sie_dfmp2_cluster_t* clusters, void* wor
             SIE_CUDA(cudaMemcpyAsync(ws + off_tiles, tiles.data(), tiles.size() * sizeof(PairTile), cudaMemcpyHostToDevice, st));
             SIE_CUDA(cudaMemsetAsync(ws + off_tiles + tiles.size() * sizeof(PairTile), 0, 256, st));
             ProfSpan ps(prof, ST_PAIR, st);
-            bool any_small = false;
-            for (int k : order) any_small = any_small || plans[k].o <= PAIR_SMALL_STRIP_MAX_O;
             // the polling producer (sie_internal.h) as soon as a third of the batch's tile work has a warp with time to spare
             // (config 2: 49 % of the work, 480.1 -> 470.8 ms; a launch of even 128-row tiles alone loses 5 % with it)
             double cost_uneven = 0.0, cost_even = 0.0;
             for (int k : order) (pair_producer_warp(plans[k].t8) ? cost_uneven : cost_even) += plans[k].tile_cost * (double)plans[k].tiles.size();
+            const int pw = 3.0 * cost_uneven >= cost_uneven + cost_even ? 12 : 0;
+            bool any_small = false;
+            for (int k : order) any_small = any_small || pair_small_strip(plans[k].o, pw != 0);
             SIE_TRY(launch_pair(reinterpret_cast<const PairCluster*>(ws + off_desc), reinterpret_cast<const PairTile*>(ws + off_tiles),
-                                (int)tiles.size(), ncta, tmax, (mode == 0 && any_small) ? 3 : mode, 3.0 * cost_uneven >= cost_uneven + cost_even ? 12 : 0, st));
+                                (int)tiles.size(), ncta, tmax, (mode == 0 && any_small) ? 3 : mode, pw, st));
         }
         // clusters with nocc > 128: the any-size slab/Gram route, one cluster at a time on shared scratch
         for (int k = 0; k < ncluster; ++k) {

@@ -152,7 +152,7 @@ int sie_dfmp2_energy_noalloc(int nocc, int nvir, int naux, const double* B, cons
     if (ce == cudaSuccess) ce = cudaMemsetAsync(gpart, 0, slot_bytes, st);
     if (ce != cudaSuccess) return set_cuda_error(ce);
     rc = launch_pair(reinterpret_cast<const PairCluster*>(base + off_desc), reinterpret_cast<const PairTile*>(base + off_tiles), (int)ntiles,
-                     ncta, t8, o <= PAIR_SMALL_STRIP_MAX_O ? 3 : 0, pair_producer_warp(t8), st);
+                     ncta, t8, pair_small_strip(o, pair_producer_warp(t8) != 0) ? 3 : 0, pair_producer_warp(t8), st);
     if (rc != SIE_OK) return rc;
     return launch_reduce(reinterpret_cast<const ReduceCluster*>(base + off_rc), 1, st);
 }

@@ -75,6 +75,11 @@ PairGeom pair_geom();
 // are epilogue_strip_small (launch_pair mode 3).  Measured (custom:o,4o,1536): small strips +4...5.5 % at o = 72...96,
 // -1 % at 104, -5 % at 112, -6 % at 120, equal at 128 — so larger blocks keep the generic strip in either instantiation.
 constexpr int PAIR_SMALL_STRIP_MAX_O = 96;
+// In the polling-producer kernels (pair_producer_warp() != 0) the small strips also win above 96: the loss at o = 104...120 came
+// from the strips' timing delaying warp 0, the producer AND pace-setter of the old placement; with the producer on warp 12
+// config 3 (o = 120) goes 0.928 -> 0.940 with them, o = 104 +1.5 %, o = 112 +-0.
+constexpr int PAIR_SMALL_STRIP_MAX_O_POLL = 120;
+inline bool pair_small_strip(int o, bool poll) { return o <= (poll ? PAIR_SMALL_STRIP_MAX_O_POLL : PAIR_SMALL_STRIP_MAX_O); }
 size_t pair_smem_bytes();
 // mode: 0 energy path (G), 1 occupied 1-RDM block (Gamma), 2 energy only with a low-rank projector, 3 = mode 0 through the
 // instantiation whose strips for o <= 64 are epilogue_strip_small (same sums; chosen by the caller when such clusters exist); one mode per launch

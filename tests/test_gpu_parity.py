@@ -104,7 +104,9 @@ RAGGED = [
     (72, 75, 0, 90),
     (81, 40, 1, 70),   # 11 strips: small-strip epilogue, o not a multiple of 8
     (96, 50, 0, 64),   # 12 strips: the largest block on the small-strip epilogue
-    (97, 30, 0, 40),   # 13 strips: first size on the generic strip
+    (97, 30, 0, 40),   # 13 strips, 104-row tiles: polling-producer kernel, small strip
+    (110, 20, 0, 40),  # 14 strips, 112-row tiles
+    (121, 12, 0, 24),  # 16 strips, 128-row tiles: warp-0 producer, generic strip
     (120, 140, 0, 200),
     (128, 130, 4, 72),
     # many virtual blocks per tile (ta = 64, 42, 18, 4 with a ragged last block), one block of 127 rows
